@@ -1,0 +1,194 @@
+/* axg.h -- C-ABI boundary of the B200-native axon-guidance time step.
+ *
+ * One `axg_step` = one pass of the per-timestep hot path of the cue-diffusion guidance model of
+ * arxiv/paper_1405_3331, as fixed by BASELINE.json `north_star` (NS) and SURVEY.md §8:
+ *   P1 Brownian diffusion of cue particles + emission at sources + absorbing-boundary removal, compacted
+ *      in order                                     (§3.5 "integration"; NS (1))
+ *   P2 uniform-grid binning: linear cell key, stable LSD radix sort of (key, index), SoA reorder,
+ *      cellStart / cellEnd                           (§3.5, Table 1; NS (2))
+ *   P3 growth-cone sensing: per-species counts and integer first moments over the cells within the
+ *      sensing radius                                (§3.5; NS (3))
+ *   P4 cone advance along the normalised gradient + seeded angular noise at fixed speed
+ *                                                    (NS (4))
+ *   P5 append of the new segment to the axon polyline, arrival / exit test
+ *                                                    (§3.4, §3.3; NS (5))
+ * The exact arithmetic (Philox keying, uniform mapping, Box-Muller pairing, stencil, tie order ...) is the
+ * list of readings in DESIGN.md §3; every kernel follows it and tests/ checks it against oracle/.
+ *
+ * Conventions
+ *  - Every pointer argument is a HOST pointer owned by the caller unless it says "device".  The library copies;
+ *    it never keeps a caller pointer after the call returns.
+ *  - The ctx owns all device memory.  One ctx is used from one host thread at a time.  No global state.
+ *  - All work is enqueued on the ctx stream (default: the legacy default stream; see axg_set_stream).
+ *  - Every call returns 0 (AXG_OK) or a negative error code; axg_last_error() gives a message.  A call that
+ *    fails with AXG_EINVAL / AXG_ECAPACITY / AXG_ESTATE / AXG_ESMALL has changed nothing.
+ *  - There is NO CPU fallback: without a CUDA device axg_create fails with AXG_ECUDA.
+ */
+#ifndef AXG_H
+#define AXG_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct axg_ctx axg_ctx; /* opaque */
+
+/* Unit cells; the domain is [0,nx) x [0,ny) x [0,nz) in cell units ("uniform grid", cell size 1). */
+typedef struct axg_grid {
+    uint32_t nx, ny, nz;
+} axg_grid;
+
+enum {
+    AXG_OK = 0,
+    AXG_EINVAL = -1,    /* bad argument (null, NaN, out of the domain, radius not in [1,8], cells >= 2^32 ...)   */
+    AXG_ECAPACITY = -2, /* particle or polyline capacity would overflow (checked on host bounds before launch) */
+    AXG_ESTATE = -3,    /* call not allowed in this state (neurons placed after the first step)                */
+    AXG_ECUDA = -4,     /* CUDA runtime error, or no device                                                    */
+    AXG_ESMALL = -5     /* dst_bytes too small; *n_elems holds the element count required                      */
+};
+
+#define AXG_MAX_SPECIES 4u
+#define AXG_MAX_SOURCES 4096u
+#define AXG_R_CAPTURE 1.0f /* arrival radius in cells (reading A-16) */
+
+/* cone state */
+enum { AXG_CONE_ACTIVE = 0, AXG_CONE_ARRIVED = 1, AXG_CONE_EXITED = 2 };
+
+/* phases for axg_step_phase */
+enum {
+    AXG_PHASE_DIFFUSE = 1, /* P1: diffuse, absorb, compact, emit, key (+ digit histograms)           */
+    AXG_PHASE_BIN = 2,     /* P2: sort, reorder, cellStart/cellEnd                                   */
+    AXG_PHASE_SENSE = 4,   /* P3                                                                     */
+    AXG_PHASE_ADVANCE = 8, /* P4 + P5                                                                */
+    AXG_PHASE_COMMIT = 16, /* step counter t += 1                                                    */
+    AXG_PHASE_ALL = 31
+};
+
+/* fields for axg_read_state.  "sorted order" = the particle array left by P2 (input of the next P1).
+ * "pre-sort" = the array written by P1 (survivors in input order, then newborns), input of P2.         */
+enum {
+    AXG_COUNTERS = 0,     /* u64[8]: step, n_live, next_id, emitted, absorbed, active, arrived, exited  */
+    AXG_PART_X = 1,       /* f32[n_live]  sorted order                                                  */
+    AXG_PART_Y = 2,
+    AXG_PART_Z = 3,
+    AXG_PART_SPECIES = 4, /* u8[n_live]                                                                 */
+    AXG_PART_ID = 5,      /* u32[n_live]                                                                */
+    AXG_KEYS_SORTED = 6,  /* u32[n_live]                                                                */
+    AXG_PERM = 7,         /* u32[n_live]  sorted j -> pre-sort index                                    */
+    AXG_CELL_START = 8,   /* u32[cells]   first sorted j of the cell, 0 if empty                        */
+    AXG_CELL_END = 9,     /* u32[cells]   one past the last sorted j, 0 if empty                        */
+    AXG_CONE_POS = 10,    /* f32[C*3] AoS                                                               */
+    AXG_CONE_HEADING = 11,/* f32[C*3] AoS                                                               */
+    AXG_CONE_STATE = 12,  /* u8[C]                                                                      */
+    AXG_CONE_COUNTS = 13, /* i64[C*AXG_MAX_SPECIES]      n_s of the last P3 in which the cone was active */
+    AXG_CONE_MOMENT = 14, /* i64[C*AXG_MAX_SPECIES*3]    M_s                                            */
+    AXG_CONE_GRADIENT = 15,/* f32[C*3]  g = G / S2(R)                                                   */
+    AXG_POLY_LEN = 16,    /* u32[C]                                                                     */
+    AXG_POLYLINE = 17,    /* f32[C*(max_segments+1)*3] neuron-major; entries >= poly_len are 0          */
+    AXG_PRE_X = 18,       /* f32[n_live]  pre-sort array (valid after P1 of the current step)           */
+    AXG_PRE_Y = 19,
+    AXG_PRE_Z = 20,
+    AXG_PRE_SPECIES = 21,
+    AXG_PRE_ID = 22,
+    AXG_PRE_KEY = 23,     /* u32[n_live]  cell key of the pre-sort array                                */
+    AXG_FIELD_COUNT = 24
+};
+
+/* Create a context on the current CUDA device.
+ *  grid      unit-cell grid, nx*ny*nz < 2^32, each >= 1
+ *  D         diffusion coefficient in cell^2/step; per-axis Gaussian step sigma = sqrt(2 D) (NS (1), config C1/C4)
+ *  emission  default particles per step per source (used when axg_add_source rate == 0)
+ *  radius    sensing radius R in cells, 1 <= R <= 8; stencil = {d in Z^3 : |d|^2 <= floor(R^2)} (A-11)
+ *  speed     cone advance per step in cells, > 0 ("a predefined distance is traversed")
+ *  noise     standard deviation (rad, small-angle) of the Gaussian heading noise, >= 0 (NS (4))
+ *  seed      Philox key = (seed low 32 bits, seed high 32 bits)
+ * Default capacities: 2^20 particles, 1024 polyline segments per cone (axg_set_capacity changes them).     */
+int axg_create(const axg_grid* grid, float D, uint32_t emission, float radius, float speed, float noise,
+               uint64_t seed, axg_ctx** out);
+
+/* Place n neurons, i.e. their growth cones (one axon per neuron, growing from the neuron).
+ *  xyz      n*3 floats AoS, each inside the domain
+ *  heading  n*3 floats AoS (normalised by the library) or NULL => (0,0,1)
+ * Replaces any neurons placed before.  Sets poly[c][0] = xyz[c], poly_len = 1, state ACTIVE.
+ * AXG_ESTATE after the first step.                                                                       */
+int axg_place_neurons(axg_ctx* ctx, const float* xyz, const float* heading, uint32_t n);
+
+/* Add a cue source ("particle systems ... placed", "particles are generated").
+ *  (x,y,z) inside the domain; species < AXG_MAX_SPECIES; polarity +1 attract / -1 repel, fixed
+ *  per species by the first source of that species (conflict => AXG_EINVAL); rate particles/step, 0 => default.
+ * Attractive sources are the arrival targets.  Allowed at any time; emits from the next step on.         */
+int axg_add_source(axg_ctx* ctx, float x, float y, float z, uint8_t species, int8_t polarity, uint32_t rate);
+
+/* Run n whole time steps (P1..P5 + commit each) on the device without host synchronisation in between;
+ * returns after the stream has been synchronised and the device error word read.                         */
+int axg_step(axg_ctx* ctx, uint32_t n);
+
+/* Copy one field to host memory.  If dst == NULL or dst_bytes is too small: returns AXG_ESMALL (or AXG_OK when
+ * dst == NULL and dst_bytes == 0) with *n_elems = number of elements of the field.  Synchronises the stream. */
+int axg_read_state(axg_ctx* ctx, uint32_t field, void* dst, size_t dst_bytes, size_t* n_elems);
+
+void axg_destroy(axg_ctx* ctx);
+
+/* Message of the last failing call on this ctx (ctx-owned, valid until the next call); with ctx == NULL the
+ * message of the last failing axg_create of this thread.                                                 */
+const char* axg_last_error(const axg_ctx* ctx);
+
+/* ---- harness / plumbing calls (not part of the paper's problem statement) ------------------------------- */
+
+/* Re-allocate for at most max_particles live particles and max_segments appended segments per cone.
+ * Keeps sources and neurons; live particles are kept if they fit, else AXG_ECAPACITY.                     */
+int axg_set_capacity(axg_ctx* ctx, uint64_t max_particles, uint32_t max_segments);
+
+/* Replace the particle array (taken as the "sorted order" array, i.e. the input of the next P1) and the id /
+ * step counters.  No validation of positions beyond n <= capacity.                                       */
+int axg_load_particles(axg_ctx* ctx, const float* x, const float* y, const float* z, const uint8_t* species,
+                       const uint32_t* id, uint64_t n, uint32_t next_id, uint32_t step);
+
+/* Replace cone position / heading / state / polyline length of the n placed cones (n must equal the placed
+ * count).  Polyline contents are kept; entry poly_len-1 is set to pos.                                    */
+int axg_load_cones(axg_ctx* ctx, const float* pos, const float* heading, const uint8_t* state,
+                   const uint32_t* poly_len, uint32_t n);
+
+/* Run the selected phases of ONE step (for per-phase parity).  AXG_PHASE_BIN without AXG_PHASE_DIFFUSE first
+ * takes the current particle array as the pre-sort array (copy + re-key), so that binning can be checked on
+ * positions produced elsewhere.  Synchronises.                                                           */
+int axg_step_phase(axg_ctx* ctx, uint32_t phase_mask);
+
+/* Multi-GPU sharding by source: this rank emits only sources with index % world == rank; the
+ * others still consume their particle ids, so trajectories equal the 1-GPU run.  Default (0,1).           */
+int axg_set_shard(axg_ctx* ctx, uint32_t rank, uint32_t world);
+
+/* Device pointer (int32[C][AXG_MAX_SPECIES][4] = n,Mx,My,Mz) of the per-cone sensing sums, for the NCCL
+ * all-reduce between P3 and P4 when sharded.  *bytes = its size.  Owned by ctx.                           */
+int axg_sense_buffer(axg_ctx* ctx, void** device_ptr, size_t* bytes);
+
+/* Use `stream` (a cudaStream_t) for all later work of this ctx.                                          */
+int axg_set_stream(axg_ctx* ctx, void* stream);
+
+/* Device-memory hooks: alloc(bytes, stream, user) -> device pointer or NULL, free(ptr, user).  Process-wide,
+ * must be set before axg_create; NULL restores cudaMalloc / cudaFree.  The Python binding routes these to the
+ * PyTorch caching allocator (NS: "PyTorch is used only for device memory and streams").                  */
+typedef void* (*axg_alloc_fn)(size_t bytes, void* stream, void* user);
+typedef void (*axg_free_fn)(void* ptr, void* user);
+int axg_set_allocator(axg_alloc_fn alloc, axg_free_fn free_, void* user);
+
+/* Timing of the last axg_step call: device milliseconds between the first and last kernel (CUDA events on the
+ * ctx stream), kernels launched, and the sum over its steps of the live particle count entering each step.  */
+int axg_last_step_stats(axg_ctx* ctx, float* device_ms, uint64_t* launches, uint64_t* particle_steps);
+
+/* Per-kernel device time of the NEXT axg_step call (debug; inserts events between kernels).  times_ms must
+ * hold AXG_KERNEL_COUNT floats after the call via axg_kernel_times.                                      */
+enum {
+    AXG_K_CLEAR = 0, AXG_K_DIFFUSE = 1, AXG_K_EMIT = 2, AXG_K_SORT = 3, AXG_K_REORDER = 4, AXG_K_SENSE = 5,
+    AXG_K_ADVANCE = 6, AXG_K_COMMIT = 7, AXG_KERNEL_COUNT = 8
+};
+int axg_profile_next_step(axg_ctx* ctx, int enable);
+int axg_kernel_times(axg_ctx* ctx, float* times_ms /* AXG_KERNEL_COUNT */);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AXG_H */
