@@ -1,0 +1,767 @@
+// axg_api.cu -- the C-ABI of include/axg.h: context, device memory, and the per-step kernel sequence.
+// Host orchestration only: every step of the path (P1..P5) runs in the kernels of axg_k_*.cu; there is no CPU
+// fallback (axg_create fails with AXG_ECUDA without a device).
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/axg.h"
+#include "axg_dev.cuh"
+
+#define AXG_API extern "C" __attribute__((visibility("default")))
+
+namespace {
+
+axg_alloc_fn g_alloc = nullptr;
+axg_free_fn g_free = nullptr;
+void* g_alloc_user = nullptr;
+thread_local std::string g_create_err;
+
+struct Source {
+    float x, y, z;
+    uint8_t species;
+    int8_t polarity;
+    uint32_t rate;
+};
+
+constexpr int N_SM = 148;
+
+}  // namespace
+
+struct axg_ctx {
+    axg_grid grid;
+    float D, radius, speed, noise;
+    uint32_t emission;
+    uint64_t seed;
+    uint64_t max_particles = 1ull << 20;
+    uint32_t max_segments = 1024;
+    uint32_t shard_rank = 0, shard_world = 1;
+    std::vector<Source> sources;
+    int8_t species_polarity[AXG_MAX_SPECIES] = {0, 0, 0, 0};
+    uint32_t n_cones = 0;
+    bool stepped = false;
+    cudaStream_t stream = nullptr;
+    std::string err;
+
+    // device memory
+    bool particles_allocated = false;
+    std::vector<void*> particle_bufs;  // everything sized by max_particles
+    void* d_dev = nullptr;
+    void* d_cell_lo = nullptr;
+    void* d_src = nullptr;
+    void* d_src_id_prefix = nullptr;
+    void* d_src_emit_prefix = nullptr;
+    void* d_stencil = nullptr;
+    std::vector<void*> cone_bufs;
+    void* d_poly = nullptr;
+    AxgParams P;
+    uint32_t loaded_species_mask = 0;  // species seen by axg_load_particles
+    uint32_t n_A = 0, n_B = 0;  // element counts of the sorted / pre-sort arrays as of the last synchronised call
+
+    // stats of the last axg_step
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    float last_ms = 0.f;
+    uint64_t last_launches = 0, last_particle_steps = 0;
+    bool profile_next = false;
+    float ktimes[AXG_KERNEL_COUNT] = {0};
+    std::vector<cudaEvent_t> prof_events;
+
+    size_t cells() const { return (size_t)grid.nx * grid.ny * grid.nz; }
+};
+
+namespace {
+
+int fail(axg_ctx* c, int code, const std::string& msg) {
+    if (c) c->err = msg; else g_create_err = msg;
+    return code;
+}
+
+int cuda_fail(axg_ctx* c, cudaError_t e, const char* what) {
+    return fail(c, AXG_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+#define CU(c, call)                                            \
+    do {                                                       \
+        cudaError_t e_ = (call);                               \
+        if (e_ != cudaSuccess) return cuda_fail(c, e_, #call); \
+    } while (0)
+
+void* dev_alloc(axg_ctx* c, size_t bytes) {
+    if (bytes == 0) bytes = 16;
+    bytes = (bytes + 255) & ~(size_t)255;
+    void* p = nullptr;
+    if (g_alloc) {
+        p = g_alloc(bytes, (void*)c->stream, g_alloc_user);
+    } else if (cudaMalloc(&p, bytes) != cudaSuccess) {
+        p = nullptr;
+    }
+    return p;
+}
+
+void dev_free(void* p) {
+    if (!p) return;
+    if (g_free) g_free(p, g_alloc_user); else cudaFree(p);
+}
+
+bool inside(const axg_ctx* c, float x, float y, float z) {
+    return x >= 0.0f && x < (float)c->grid.nx && y >= 0.0f && y < (float)c->grid.ny && z >= 0.0f &&
+           z < (float)c->grid.nz;
+}
+
+uint64_t owned_rate(const axg_ctx* c) {
+    uint64_t e = 0;
+    for (size_t s = 0; s < c->sources.size(); ++s)
+        if (s % c->shard_world == c->shard_rank) e += c->sources[s].rate;
+    return e;
+}
+
+int key_passes(size_t cells) {
+    int bits = 1;
+    while (bits < 32 && ((size_t)1 << bits) < cells) ++bits;
+    return (bits + 7) / 8;
+}
+
+// ---- allocation ------------------------------------------------------------------------------------------
+int alloc_fixed(axg_ctx* c) {
+    if (c->d_dev) return AXG_OK;
+    c->d_dev = dev_alloc(c, sizeof(AxgDev));
+    c->d_cell_lo = dev_alloc(c, (c->cells() + 1) * sizeof(uint32_t));
+    c->d_src = dev_alloc(c, AXG_MAX_SOURCES * sizeof(AxgSourceDev));
+    c->d_src_id_prefix = dev_alloc(c, (AXG_MAX_SOURCES + 1) * sizeof(uint32_t));
+    c->d_src_emit_prefix = dev_alloc(c, (AXG_MAX_SOURCES + 1) * sizeof(uint32_t));
+    // stencil {d : |d|^2 <= floor(R^2)} (reading A-11) and S2(R) = sum dx^2 (reading A-12)
+    const int r2 = (int)std::floor((double)c->radius * (double)c->radius);
+    const int R = (int)std::floor((double)c->radius);
+    std::vector<int32_t> st;
+    long long s2 = 0;
+    for (int dz = -R; dz <= R; ++dz)
+        for (int dy = -R; dy <= R; ++dy)
+            for (int dx = -R; dx <= R; ++dx)
+                if (dx * dx + dy * dy + dz * dz <= r2) {
+                    st.push_back((dx & 0xff) | ((dy & 0xff) << 8) | ((dz & 0xff) << 16));
+                    s2 += dx * dx;
+                }
+    c->d_stencil = dev_alloc(c, st.size() * sizeof(int32_t));
+    if (!c->d_dev || !c->d_cell_lo || !c->d_src || !c->d_src_id_prefix || !c->d_src_emit_prefix || !c->d_stencil)
+        return fail(c, AXG_ECUDA, "device allocation failed");
+    CU(c, cudaMemsetAsync(c->d_dev, 0, sizeof(AxgDev), c->stream));
+    CU(c, cudaMemsetAsync(c->d_cell_lo, 0, (c->cells() + 1) * sizeof(uint32_t), c->stream));
+    CU(c, cudaMemcpyAsync(c->d_stencil, st.data(), st.size() * sizeof(int32_t), cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    AxgParams& P = c->P;
+    P.dev = (AxgDev*)c->d_dev;
+    P.cell_lo = (uint32_t*)c->d_cell_lo;
+    P.nx = c->grid.nx; P.ny = c->grid.ny; P.nz = c->grid.nz; P.cells = (uint32_t)c->cells();
+    P.fnx = (float)c->grid.nx; P.fny = (float)c->grid.ny; P.fnz = (float)c->grid.nz;
+    P.sigma = (float)std::sqrt(2.0 * (double)c->D);  // O0
+    P.seed_lo = (uint32_t)(c->seed & 0xffffffffull);
+    P.seed_hi = (uint32_t)(c->seed >> 32);
+    P.n_pass = key_passes(c->cells());
+    P.final_buf = (P.n_pass - 1) & 1;
+    P.src = (const AxgSourceDev*)c->d_src;
+    P.src_id_prefix = (const uint32_t*)c->d_src_id_prefix;
+    P.src_emit_prefix = (const uint32_t*)c->d_src_emit_prefix;
+    P.stencil = (const int32_t*)c->d_stencil;
+    P.n_stencil = (uint32_t)st.size();
+    P.s2 = (float)s2;
+    P.speed = c->speed; P.noise = c->noise;
+    return AXG_OK;
+}
+
+void free_particles(axg_ctx* c) {
+    for (void* p : c->particle_bufs) dev_free(p);
+    c->particle_bufs.clear();
+    c->particles_allocated = false;
+}
+
+// fills P.A, P.B, keys, look-back words for `cap` particles
+int alloc_particles(axg_ctx* c, uint64_t cap, AxgParams& P, std::vector<void*>& bufs) {
+    const size_t pad = 64;  // tail padding so that ragged tiles may over-read harmlessly
+    const size_t n = (size_t)cap + pad;
+    const size_t diff_tiles = n / axg_diffuse_tile() + 2, sort_tiles = n / axg_sort_tile() + 2;
+    const size_t sizes[] = {n * 4, n * 4, n * 4, n, n * 4,  // A
+                            n * 4, n * 4, n * 4, n, n * 4,  // B
+                            n * 4, n * 4, n * 4, n * 4, n * 4,  // key_pre, skey[2], sidx[2]
+                            diff_tiles * 8, sort_tiles * AXG_RADIX * 8};
+    void* ptr[17];
+    for (int i = 0; i < 17; ++i) {
+        ptr[i] = dev_alloc(c, sizes[i]);
+        if (!ptr[i]) {
+            for (int k = 0; k < i; ++k) dev_free(ptr[k]);
+            bufs.resize(bufs.size() - (size_t)i);
+            return fail(c, AXG_ECUDA, "device allocation failed (particle arrays)");
+        }
+        bufs.push_back(ptr[i]);
+    }
+    P.A = AxgSoA{(float*)ptr[0], (float*)ptr[1], (float*)ptr[2], (uint8_t*)ptr[3], (uint32_t*)ptr[4]};
+    P.B = AxgSoA{(float*)ptr[5], (float*)ptr[6], (float*)ptr[7], (uint8_t*)ptr[8], (uint32_t*)ptr[9]};
+    P.key_pre = (uint32_t*)ptr[10];
+    P.skey[0] = (uint32_t*)ptr[11]; P.skey[1] = (uint32_t*)ptr[12];
+    P.sidx[0] = (uint32_t*)ptr[13]; P.sidx[1] = (uint32_t*)ptr[14];
+    P.tile_state = (unsigned long long*)ptr[15];
+    P.sort_state = (unsigned long long*)ptr[16];
+    P.capacity = (uint32_t)cap;
+    // look-back words must not alias a live epoch: zero them (epoch 0 words with flag 0 = not ready)
+    CU(c, cudaMemsetAsync(ptr[15], 0, sizes[15], c->stream));
+    CU(c, cudaMemsetAsync(ptr[16], 0, sizes[16], c->stream));
+    return AXG_OK;
+}
+
+int ensure_particles(axg_ctx* c) {
+    int rc = alloc_fixed(c);
+    if (rc) return rc;
+    if (c->particles_allocated) return AXG_OK;
+    rc = alloc_particles(c, c->max_particles, c->P, c->particle_bufs);
+    if (rc) return rc;
+    c->particles_allocated = true;
+    return AXG_OK;
+}
+
+void free_cones(axg_ctx* c) {
+    for (void* p : c->cone_bufs) dev_free(p);
+    c->cone_bufs.clear();
+    dev_free(c->d_poly);
+    c->d_poly = nullptr;
+}
+
+size_t poly_bytes(const axg_ctx* c, uint32_t max_segments) {
+    return ((size_t)max_segments + 1) * 3 * (size_t)c->n_cones * sizeof(float);
+}
+
+int alloc_cones(axg_ctx* c, uint32_t n) {
+    free_cones(c);
+    c->n_cones = n;
+    AxgParams& P = c->P;
+    P.n_cones = n;
+    P.max_segments = c->max_segments;
+    if (n == 0) return AXG_OK;
+    const size_t sizes[] = {(size_t)n * 12, (size_t)n * 12, (size_t)n, (size_t)n * 64, (size_t)n * 12, (size_t)n * 4};
+    void* ptr[6];
+    for (int i = 0; i < 6; ++i) {
+        ptr[i] = dev_alloc(c, sizes[i]);
+        if (!ptr[i]) return fail(c, AXG_ECUDA, "device allocation failed (cones)");
+        c->cone_bufs.push_back(ptr[i]);
+        CU(c, cudaMemsetAsync(ptr[i], 0, sizes[i], c->stream));
+    }
+    c->d_poly = dev_alloc(c, poly_bytes(c, c->max_segments));
+    if (!c->d_poly) return fail(c, AXG_ECUDA, "device allocation failed (polylines)");
+    CU(c, cudaMemsetAsync(c->d_poly, 0, poly_bytes(c, c->max_segments), c->stream));
+    P.cone_pos = (float*)ptr[0]; P.cone_heading = (float*)ptr[1]; P.cone_state = (uint8_t*)ptr[2];
+    P.sense = (int32_t*)ptr[3]; P.cone_gradient = (float*)ptr[4]; P.poly_len = (uint32_t*)ptr[5];
+    P.poly = (float*)c->d_poly;
+    return AXG_OK;
+}
+
+// upload sources + the two rate prefixes, refresh the source-derived parameters
+int upload_sources(axg_ctx* c) {
+    int rc = alloc_fixed(c);
+    if (rc) return rc;
+    const size_t S = c->sources.size();
+    std::vector<AxgSourceDev> sd(S);
+    std::vector<uint32_t> idp(S + 1, 0u), emp(S + 1, 0u);
+    int n_species_used = 0, only = -1;
+    for (int s = 0; s < (int)AXG_MAX_SPECIES; ++s) {
+        c->P.polarity[s] = c->species_polarity[s];
+        if (c->species_polarity[s] != 0 || ((c->loaded_species_mask >> s) & 1u)) { ++n_species_used; only = s; }
+    }
+    for (size_t s = 0; s < S; ++s) {
+        const Source& q = c->sources[s];
+        sd[s] = AxgSourceDev{q.x, q.y, q.z, (uint32_t)q.species | (q.polarity == 1 ? 0x100u : 0u)};
+        const bool owned = (s % c->shard_world) == c->shard_rank;
+        idp[s + 1] = idp[s] + q.rate;
+        emp[s + 1] = emp[s] + (owned ? q.rate : 0u);
+    }
+    if (S) {
+        CU(c, cudaMemcpyAsync(c->d_src, sd.data(), S * sizeof(AxgSourceDev), cudaMemcpyHostToDevice, c->stream));
+    }
+    CU(c, cudaMemcpyAsync(c->d_src_id_prefix, idp.data(), (S + 1) * 4, cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaMemcpyAsync(c->d_src_emit_prefix, emp.data(), (S + 1) * 4, cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    c->P.n_src = (uint32_t)S;
+    c->P.e_total = idp[S];
+    c->P.e_owned = emp[S];
+    // with one species in use (by sources and by loaded particles) every particle in a cell has it: counts come
+    // from cell_lo alone and the species bytes are not walked.
+    c->P.single_species = (n_species_used == 1) ? only : -1;
+    return AXG_OK;
+}
+
+int read_dev(axg_ctx* c, AxgDev* h) {
+    CU(c, cudaMemcpyAsync(h, c->d_dev, sizeof(AxgDev), cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    return AXG_OK;
+}
+
+}  // namespace
+
+// ============================================ step sequence ==================================================
+namespace {
+
+struct Prof {
+    axg_ctx* c;
+    bool on;
+    size_t used = 0;
+    std::vector<int> tags;
+    void mark(int tag) {  // event BEFORE the kernel(s) of `tag`; a final mark(-1) closes the last one
+        if (!on) return;
+        if (used == c->prof_events.size()) {
+            cudaEvent_t e;
+            cudaEventCreate(&e);
+            c->prof_events.push_back(e);
+        }
+        cudaEventRecord(c->prof_events[used++], c->stream);
+        tags.push_back(tag);
+    }
+};
+
+// enqueue the selected phases of one step; returns the number of kernel launches
+int enqueue_phases(axg_ctx* c, uint32_t mask, Prof& prof) {
+    const AxgParams& P = c->P;
+    cudaStream_t s = c->stream;
+    int launches = 0;
+    if (mask & AXG_PHASE_DIFFUSE) {
+        prof.mark(AXG_K_DIFFUSE);
+        axg_launch_diffuse(P, N_SM * 3, s);
+        prof.mark(AXG_K_EMIT);
+        axg_launch_emit(P, 1, s);
+        launches += 2;
+    }
+    if (mask & AXG_PHASE_BIN) {
+        if (!(mask & AXG_PHASE_DIFFUSE)) {
+            prof.mark(AXG_K_EMIT);
+            axg_launch_rekey(P, N_SM * 8, s);
+            axg_launch_emit(P, 0, s);
+            launches += 2;
+        }
+        prof.mark(AXG_K_SORT);
+        for (int q = 0; q < P.n_pass; ++q) axg_launch_sort_pass(P, q, N_SM * 2, s);
+        prof.mark(AXG_K_REORDER);
+        axg_launch_reorder(P, N_SM * 8, s);
+        launches += P.n_pass + 1;
+    }
+    if ((mask & AXG_PHASE_SENSE) && P.n_cones) {
+        prof.mark(AXG_K_SENSE);
+        axg_launch_sense(P, s);
+        launches += 1;
+    }
+    if ((mask & AXG_PHASE_ADVANCE) && P.n_cones) {
+        prof.mark(AXG_K_ADVANCE);
+        axg_launch_advance(P, s);
+        launches += 1;
+    }
+    if (mask & AXG_PHASE_COMMIT) {
+        prof.mark(AXG_K_COMMIT);
+        axg_launch_commit(P, s);
+        launches += 1;
+    }
+    return launches;
+}
+
+void finish_prof(axg_ctx* c, Prof& prof) {
+    if (!prof.on) return;
+    for (int k = 0; k < AXG_KERNEL_COUNT; ++k) c->ktimes[k] = 0.f;
+    for (size_t i = 0; i + 1 < prof.used; ++i) {
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, c->prof_events[i], c->prof_events[i + 1]);
+        if (prof.tags[i] >= 0) c->ktimes[prof.tags[i]] += ms;
+    }
+}
+
+// host-side pre-checks from device counters: nothing is enqueued when they fail
+int capacity_check(axg_ctx* c, uint32_t n, bool diffuse, bool advance, AxgDev* h) {
+    int rc = read_dev(c, h);
+    if (rc) return rc;
+    if (diffuse && (uint64_t)h->n_live + (uint64_t)n * owned_rate(c) > c->max_particles)
+        return fail(c, AXG_ECAPACITY, "particle capacity would overflow");
+    if (advance && c->n_cones) {
+        CU(c, cudaMemsetAsync(&((AxgDev*)c->d_dev)->cone_census[0], 0, 4 * sizeof(uint32_t), c->stream));
+        axg_launch_census(c->P, c->stream);
+        rc = read_dev(c, h);
+        if (rc) return rc;
+        if (h->cone_census[0] && (uint64_t)h->cone_census[3] + n > (uint64_t)c->max_segments + 1)
+            return fail(c, AXG_ECAPACITY, "polyline capacity would overflow");
+    }
+    return AXG_OK;
+}
+
+int after_sync(axg_ctx* c, const char* what) {
+    cudaError_t e = cudaStreamSynchronize(c->stream);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(c, e, what);
+    return AXG_OK;
+}
+
+}  // namespace
+
+// ============================================ exported ABI ===================================================
+
+AXG_API int axg_set_allocator(axg_alloc_fn alloc, axg_free_fn free_, void* user) {
+    if ((alloc == nullptr) != (free_ == nullptr)) return AXG_EINVAL;
+    g_alloc = alloc; g_free = free_; g_alloc_user = user;
+    return AXG_OK;
+}
+
+AXG_API int axg_create(const axg_grid* grid, float D, uint32_t emission, float radius, float speed, float noise,
+                       uint64_t seed, axg_ctx** out) {
+    if (!grid || !out) return fail(nullptr, AXG_EINVAL, "null argument");
+    if (grid->nx == 0 || grid->ny == 0 || grid->nz == 0) return fail(nullptr, AXG_EINVAL, "empty grid");
+    if ((double)grid->nx * grid->ny * grid->nz >= 4294967296.0) return fail(nullptr, AXG_EINVAL, "cells >= 2^32");
+    if (!(D >= 0.0f) || !(radius >= 1.0f && radius <= 8.0f) || !(speed > 0.0f) || !(noise >= 0.0f) ||
+        !std::isfinite(D) || !std::isfinite(speed) || !std::isfinite(noise))
+        return fail(nullptr, AXG_EINVAL, "bad D / radius / speed / noise");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(nullptr, AXG_ECUDA, "no CUDA device: this library has no CPU fallback");
+    }
+    axg_ctx* c = new axg_ctx();
+    c->grid = *grid;
+    c->D = D; c->emission = emission; c->radius = radius; c->speed = speed; c->noise = noise; c->seed = seed;
+    std::memset(&c->P, 0, sizeof(c->P));
+    c->P.single_species = -1;
+    *out = c;
+    return AXG_OK;
+}
+
+AXG_API void axg_destroy(axg_ctx* c) {
+    if (!c) return;
+    cudaStreamSynchronize(c->stream);
+    free_particles(c);
+    free_cones(c);
+    dev_free(c->d_dev); dev_free(c->d_cell_lo); dev_free(c->d_src); dev_free(c->d_src_id_prefix);
+    dev_free(c->d_src_emit_prefix); dev_free(c->d_stencil);
+    for (cudaEvent_t e : c->prof_events) cudaEventDestroy(e);
+    if (c->ev0) cudaEventDestroy(c->ev0);
+    if (c->ev1) cudaEventDestroy(c->ev1);
+    delete c;
+}
+
+AXG_API const char* axg_last_error(const axg_ctx* c) { return c ? c->err.c_str() : g_create_err.c_str(); }
+
+AXG_API int axg_set_stream(axg_ctx* c, void* stream) {
+    if (!c) return AXG_EINVAL;
+    cudaStreamSynchronize(c->stream);
+    c->stream = (cudaStream_t)stream;
+    return AXG_OK;
+}
+
+AXG_API int axg_set_shard(axg_ctx* c, uint32_t rank, uint32_t world) {
+    if (!c || world == 0 || rank >= world) return fail(c, AXG_EINVAL, "bad shard");
+    c->shard_rank = rank; c->shard_world = world;
+    return upload_sources(c);
+}
+
+AXG_API int axg_add_source(axg_ctx* c, float x, float y, float z, uint8_t species, int8_t polarity, uint32_t rate) {
+    if (!c) return AXG_EINVAL;
+    if (!inside(c, x, y, z)) return fail(c, AXG_EINVAL, "source outside the domain");
+    if (species >= AXG_MAX_SPECIES) return fail(c, AXG_EINVAL, "species >= 4");
+    if (polarity != 1 && polarity != -1) return fail(c, AXG_EINVAL, "polarity must be +1 or -1");
+    if (c->species_polarity[species] != 0 && c->species_polarity[species] != polarity)
+        return fail(c, AXG_EINVAL, "polarity conflict within a species");
+    if (c->sources.size() >= AXG_MAX_SOURCES) return fail(c, AXG_EINVAL, "too many sources");
+    c->species_polarity[species] = polarity;
+    c->sources.push_back(Source{x, y, z, species, polarity, rate ? rate : c->emission});
+    return upload_sources(c);
+}
+
+AXG_API int axg_place_neurons(axg_ctx* c, const float* xyz, const float* heading, uint32_t n) {
+    if (!c || (!xyz && n)) return fail(c, AXG_EINVAL, "null argument");
+    if (c->stepped) return fail(c, AXG_ESTATE, "neurons cannot be placed after the first step");
+    std::vector<float> hd((size_t)n * 3);
+    for (uint32_t i = 0; i < n; ++i) {
+        if (!inside(c, xyz[i * 3], xyz[i * 3 + 1], xyz[i * 3 + 2])) return fail(c, AXG_EINVAL, "neuron outside the domain");
+        if (heading) {
+            const float* h = &heading[i * 3];
+            const float l = std::sqrt(h[0] * h[0] + h[1] * h[1] + h[2] * h[2]);
+            if (!(l > 0.0f) || !std::isfinite(l)) return fail(c, AXG_EINVAL, "bad heading");
+            for (int a = 0; a < 3; ++a) hd[(size_t)i * 3 + a] = h[a] / l;
+        } else {  // reading A-20: default +z
+            hd[(size_t)i * 3 + 0] = 0.0f; hd[(size_t)i * 3 + 1] = 0.0f; hd[(size_t)i * 3 + 2] = 1.0f;
+        }
+    }
+    int rc = alloc_fixed(c);
+    if (rc) return rc;
+    rc = alloc_cones(c, n);
+    if (rc) return rc;
+    if (n == 0) return AXG_OK;
+    std::vector<uint32_t> ones(n, 1u);
+    CU(c, cudaMemcpyAsync(c->P.cone_pos, xyz, (size_t)n * 12, cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaMemcpyAsync(c->P.cone_heading, hd.data(), (size_t)n * 12, cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaMemcpyAsync(c->P.poly_len, ones.data(), (size_t)n * 4, cudaMemcpyHostToDevice, c->stream));
+    axg_launch_poly_init(c->P, c->stream);
+    return after_sync(c, "axg_place_neurons");
+}
+
+AXG_API int axg_set_capacity(axg_ctx* c, uint64_t max_particles, uint32_t max_segments) {
+    if (!c || max_particles == 0 || max_particles >= 0xffffff00ull) return fail(c, AXG_EINVAL, "bad capacity");
+    int rc = alloc_fixed(c);
+    if (rc) return rc;
+    AxgDev h;
+    rc = read_dev(c, &h);
+    if (rc) return rc;
+    if (h.n_live > max_particles) return fail(c, AXG_ECAPACITY, "live particles exceed the new capacity");
+    if (c->n_cones && max_segments != c->max_segments) {
+        std::vector<uint32_t> len(c->n_cones);
+        CU(c, cudaMemcpy(len.data(), c->P.poly_len, (size_t)c->n_cones * 4, cudaMemcpyDeviceToHost));
+        uint32_t longest = *std::max_element(len.begin(), len.end());
+        if (longest > (uint64_t)max_segments + 1) return fail(c, AXG_ECAPACITY, "polylines exceed the new capacity");
+        // step-major planes: a different capacity only changes the number of rows
+        void* np = dev_alloc(c, poly_bytes(c, max_segments));
+        if (!np) return fail(c, AXG_ECUDA, "device allocation failed (polylines)");
+        CU(c, cudaMemsetAsync(np, 0, poly_bytes(c, max_segments), c->stream));
+        CU(c, cudaMemcpyAsync(np, c->d_poly, std::min(poly_bytes(c, max_segments), poly_bytes(c, c->max_segments)),
+                              cudaMemcpyDeviceToDevice, c->stream));
+        CU(c, cudaStreamSynchronize(c->stream));
+        dev_free(c->d_poly);
+        c->d_poly = np;
+        c->P.poly = (float*)np;
+    }
+    c->max_segments = max_segments;
+    c->P.max_segments = max_segments;
+    if (c->particles_allocated && max_particles != c->max_particles) {
+        AxgParams NP = c->P;
+        std::vector<void*> nb;
+        rc = alloc_particles(c, max_particles, NP, nb);
+        if (rc) return rc;
+        const size_t n = h.n_live;
+        if (n) {
+            CU(c, cudaMemcpyAsync(NP.A.x, c->P.A.x, n * 4, cudaMemcpyDeviceToDevice, c->stream));
+            CU(c, cudaMemcpyAsync(NP.A.y, c->P.A.y, n * 4, cudaMemcpyDeviceToDevice, c->stream));
+            CU(c, cudaMemcpyAsync(NP.A.z, c->P.A.z, n * 4, cudaMemcpyDeviceToDevice, c->stream));
+            CU(c, cudaMemcpyAsync(NP.A.id, c->P.A.id, n * 4, cudaMemcpyDeviceToDevice, c->stream));
+            CU(c, cudaMemcpyAsync(NP.A.species, c->P.A.species, n, cudaMemcpyDeviceToDevice, c->stream));
+        }
+        CU(c, cudaStreamSynchronize(c->stream));
+        free_particles(c);
+        c->P = NP;
+        c->particle_bufs = nb;
+        c->particles_allocated = true;
+        c->n_B = 0;
+    }
+    c->max_particles = max_particles;
+    return AXG_OK;
+}
+
+AXG_API int axg_load_particles(axg_ctx* c, const float* x, const float* y, const float* z, const uint8_t* species,
+                               const uint32_t* id, uint64_t n, uint32_t next_id, uint32_t step) {
+    if (!c || (n && (!x || !y || !z || !species || !id))) return fail(c, AXG_EINVAL, "null argument");
+    if (n > c->max_particles) return fail(c, AXG_ECAPACITY, "more particles than capacity");
+    uint32_t mask = 0;
+    for (uint64_t i = 0; i < n; ++i) {
+        if (species[i] >= AXG_MAX_SPECIES) return fail(c, AXG_EINVAL, "species >= 4");
+        mask |= 1u << species[i];
+    }
+    int rc = ensure_particles(c);
+    if (rc) return rc;
+    if (n) {
+        CU(c, cudaMemcpyAsync(c->P.A.x, x, n * 4, cudaMemcpyHostToDevice, c->stream));
+        CU(c, cudaMemcpyAsync(c->P.A.y, y, n * 4, cudaMemcpyHostToDevice, c->stream));
+        CU(c, cudaMemcpyAsync(c->P.A.z, z, n * 4, cudaMemcpyHostToDevice, c->stream));
+        CU(c, cudaMemcpyAsync(c->P.A.id, id, n * 4, cudaMemcpyHostToDevice, c->stream));
+        CU(c, cudaMemcpyAsync(c->P.A.species, species, n, cudaMemcpyHostToDevice, c->stream));
+    }
+    AxgDev* d = (AxgDev*)c->d_dev;
+    const uint32_t n32 = (uint32_t)n;
+    CU(c, cudaMemcpyAsync(&d->n_live, &n32, 4, cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaMemcpyAsync(&d->next_id, &next_id, 4, cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaMemcpyAsync(&d->step, &step, 4, cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    c->n_A = n32;
+    c->loaded_species_mask = mask;
+    return upload_sources(c);
+}
+
+AXG_API int axg_load_cones(axg_ctx* c, const float* pos, const float* heading, const uint8_t* state,
+                           const uint32_t* poly_len, uint32_t n) {
+    if (!c || !pos || !heading || !state || !poly_len) return fail(c, AXG_EINVAL, "null argument");
+    if (n != c->n_cones) return fail(c, AXG_EINVAL, "cone count differs from the placed count");
+    for (uint32_t i = 0; i < n; ++i)
+        if (poly_len[i] == 0 || poly_len[i] > c->max_segments + 1) return fail(c, AXG_EINVAL, "bad poly_len");
+    if (n == 0) return AXG_OK;
+    CU(c, cudaMemcpyAsync(c->P.cone_pos, pos, (size_t)n * 12, cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaMemcpyAsync(c->P.cone_heading, heading, (size_t)n * 12, cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaMemcpyAsync(c->P.cone_state, state, (size_t)n, cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaMemcpyAsync(c->P.poly_len, poly_len, (size_t)n * 4, cudaMemcpyHostToDevice, c->stream));
+    axg_launch_poly_init(c->P, c->stream);
+    return after_sync(c, "axg_load_cones");
+}
+
+AXG_API int axg_step(axg_ctx* c, uint32_t n) {
+    if (!c) return AXG_EINVAL;
+    int rc = ensure_particles(c);
+    if (rc) return rc;
+    AxgDev h;
+    rc = capacity_check(c, n, true, true, &h);
+    if (rc) return rc;
+    if (!c->ev0) {
+        CU(c, cudaEventCreate(&c->ev0));
+        CU(c, cudaEventCreate(&c->ev1));
+    }
+    const unsigned long long ps0 = h.particle_steps;
+    Prof prof{c, c->profile_next};
+    c->profile_next = false;
+    uint64_t launches = 0;
+    CU(c, cudaEventRecord(c->ev0, c->stream));
+    for (uint32_t i = 0; i < n; ++i) launches += enqueue_phases(c, AXG_PHASE_ALL, prof);
+    prof.mark(-1);
+    CU(c, cudaEventRecord(c->ev1, c->stream));
+    c->stepped = true;
+    rc = after_sync(c, "axg_step");
+    if (rc) return rc;
+    finish_prof(c, prof);
+    cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1);
+    c->last_launches = launches;
+    rc = read_dev(c, &h);
+    if (rc) return rc;
+    c->last_particle_steps = h.particle_steps - ps0;
+    c->n_A = c->n_B = h.n_live;
+    if (h.err) {
+        char msg[96];
+        std::snprintf(msg, sizeof msg, "device error word 0x%x (1 = particle capacity, 2 = polyline capacity)", h.err);
+        return fail(c, AXG_ECAPACITY, msg);
+    }
+    return AXG_OK;
+}
+
+AXG_API int axg_step_phase(axg_ctx* c, uint32_t mask) {
+    if (!c || (mask & ~(uint32_t)AXG_PHASE_ALL)) return fail(c, AXG_EINVAL, "bad phase mask");
+    int rc = ensure_particles(c);
+    if (rc) return rc;
+    AxgDev h;
+    rc = capacity_check(c, 1, (mask & AXG_PHASE_DIFFUSE) != 0, (mask & AXG_PHASE_ADVANCE) != 0, &h);
+    if (rc) return rc;
+    Prof prof{c, false};
+    enqueue_phases(c, mask, prof);
+    c->stepped = true;
+    rc = after_sync(c, "axg_step_phase");
+    if (rc) return rc;
+    rc = read_dev(c, &h);
+    if (rc) return rc;
+    if (mask & AXG_PHASE_DIFFUSE) c->n_B = h.n_live;
+    if (mask & AXG_PHASE_BIN) c->n_A = c->n_B = h.n_live;
+    if (h.err) return fail(c, AXG_ECAPACITY, "device error word set");
+    return AXG_OK;
+}
+
+namespace {
+
+// copy `n` elements of `elem` bytes from device memory to dst, with the ESMALL protocol of axg_read_state
+int copy_out(axg_ctx* c, const void* dsrc, size_t n, size_t elem, void* dst, size_t dst_bytes, size_t* n_elems) {
+    if (n_elems) *n_elems = n;
+    if (dst == nullptr && dst_bytes == 0) return AXG_OK;
+    if (dst == nullptr || dst_bytes < n * elem) return fail(c, AXG_ESMALL, "destination too small");
+    if (n) {
+        CU(c, cudaMemcpyAsync(dst, dsrc, n * elem, cudaMemcpyDeviceToHost, c->stream));
+        CU(c, cudaStreamSynchronize(c->stream));
+    }
+    return AXG_OK;
+}
+
+// fields that are produced by a small export kernel into a scratch buffer first
+template <class Launch>
+int export_out(axg_ctx* c, size_t n, size_t elem, void* dst, size_t dst_bytes, size_t* n_elems, Launch launch) {
+    if (n_elems) *n_elems = n;
+    if (dst == nullptr && dst_bytes == 0) return AXG_OK;
+    if (dst == nullptr || dst_bytes < n * elem) return fail(c, AXG_ESMALL, "destination too small");
+    if (n == 0) return AXG_OK;
+    void* tmp = dev_alloc(c, n * elem);
+    if (!tmp) return fail(c, AXG_ECUDA, "device allocation failed (export scratch)");
+    launch(tmp);
+    cudaError_t e = cudaMemcpyAsync(dst, tmp, n * elem, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    dev_free(tmp);
+    if (e != cudaSuccess) return cuda_fail(c, e, "export");
+    return AXG_OK;
+}
+
+}  // namespace
+
+AXG_API int axg_read_state(axg_ctx* c, uint32_t field, void* dst, size_t dst_bytes, size_t* n_elems) {
+    if (!c) return AXG_EINVAL;
+    if (field >= AXG_FIELD_COUNT) return fail(c, AXG_EINVAL, "unknown field");
+    int rc = alloc_fixed(c);
+    if (rc) return rc;
+    const AxgParams& P = c->P;
+    const bool have_p = c->particles_allocated;
+    const size_t nA = have_p ? c->n_A : 0, nB = have_p ? c->n_B : 0, C = c->n_cones;
+    switch (field) {
+        case AXG_COUNTERS: {
+            if (n_elems) *n_elems = 8;
+            if (dst == nullptr && dst_bytes == 0) return AXG_OK;
+            if (dst == nullptr || dst_bytes < 64) return fail(c, AXG_ESMALL, "destination too small");
+            CU(c, cudaMemsetAsync(&((AxgDev*)c->d_dev)->cone_census[0], 0, 4 * sizeof(uint32_t), c->stream));
+            axg_launch_census(P, c->stream);
+            AxgDev h;
+            rc = read_dev(c, &h);
+            if (rc) return rc;
+            const uint64_t v[8] = {h.step, h.n_live, h.next_id, h.emitted, h.absorbed,
+                                   h.cone_census[0], h.cone_census[1], h.cone_census[2]};
+            std::memcpy(dst, v, 64);
+            return AXG_OK;
+        }
+        case AXG_PART_X: return copy_out(c, P.A.x, nA, 4, dst, dst_bytes, n_elems);
+        case AXG_PART_Y: return copy_out(c, P.A.y, nA, 4, dst, dst_bytes, n_elems);
+        case AXG_PART_Z: return copy_out(c, P.A.z, nA, 4, dst, dst_bytes, n_elems);
+        case AXG_PART_SPECIES: return copy_out(c, P.A.species, nA, 1, dst, dst_bytes, n_elems);
+        case AXG_PART_ID: return copy_out(c, P.A.id, nA, 4, dst, dst_bytes, n_elems);
+        case AXG_KEYS_SORTED: return copy_out(c, have_p ? P.skey[P.final_buf] : nullptr, nB, 4, dst, dst_bytes, n_elems);
+        case AXG_PERM: return copy_out(c, have_p ? P.sidx[P.final_buf] : nullptr, nB, 4, dst, dst_bytes, n_elems);
+        case AXG_CELL_START:
+            return export_out(c, c->cells(), 4, dst, dst_bytes, n_elems,
+                              [&](void* t) { axg_launch_cell_export(P, (uint32_t*)t, nullptr, c->stream); });
+        case AXG_CELL_END:
+            return export_out(c, c->cells(), 4, dst, dst_bytes, n_elems,
+                              [&](void* t) { axg_launch_cell_export(P, nullptr, (uint32_t*)t, c->stream); });
+        case AXG_CONE_POS: return copy_out(c, P.cone_pos, C * 3, 4, dst, dst_bytes, n_elems);
+        case AXG_CONE_HEADING: return copy_out(c, P.cone_heading, C * 3, 4, dst, dst_bytes, n_elems);
+        case AXG_CONE_STATE: return copy_out(c, P.cone_state, C, 1, dst, dst_bytes, n_elems);
+        case AXG_CONE_COUNTS:
+            return export_out(c, C * AXG_MAX_SPECIES, 8, dst, dst_bytes, n_elems,
+                              [&](void* t) { axg_launch_sense_export(P, (long long*)t, nullptr, c->stream); });
+        case AXG_CONE_MOMENT:
+            return export_out(c, C * AXG_MAX_SPECIES * 3, 8, dst, dst_bytes, n_elems,
+                              [&](void* t) { axg_launch_sense_export(P, nullptr, (long long*)t, c->stream); });
+        case AXG_CONE_GRADIENT: return copy_out(c, P.cone_gradient, C * 3, 4, dst, dst_bytes, n_elems);
+        case AXG_POLY_LEN: return copy_out(c, P.poly_len, C, 4, dst, dst_bytes, n_elems);
+        case AXG_POLYLINE:
+            return export_out(c, C * ((size_t)c->max_segments + 1) * 3, 4, dst, dst_bytes, n_elems,
+                              [&](void* t) { axg_launch_poly_export(P, (float*)t, c->stream); });
+        case AXG_PRE_X: return copy_out(c, P.B.x, nB, 4, dst, dst_bytes, n_elems);
+        case AXG_PRE_Y: return copy_out(c, P.B.y, nB, 4, dst, dst_bytes, n_elems);
+        case AXG_PRE_Z: return copy_out(c, P.B.z, nB, 4, dst, dst_bytes, n_elems);
+        case AXG_PRE_SPECIES: return copy_out(c, P.B.species, nB, 1, dst, dst_bytes, n_elems);
+        case AXG_PRE_ID: return copy_out(c, P.B.id, nB, 4, dst, dst_bytes, n_elems);
+        case AXG_PRE_KEY: return copy_out(c, P.key_pre, nB, 4, dst, dst_bytes, n_elems);
+        default: return fail(c, AXG_EINVAL, "unknown field");
+    }
+}
+
+AXG_API int axg_sense_buffer(axg_ctx* c, void** device_ptr, size_t* bytes) {
+    if (!c || !device_ptr || !bytes) return AXG_EINVAL;
+    *device_ptr = c->n_cones ? (void*)c->P.sense : nullptr;
+    *bytes = (size_t)c->n_cones * 16 * sizeof(int32_t);
+    return AXG_OK;
+}
+
+AXG_API int axg_last_step_stats(axg_ctx* c, float* device_ms, uint64_t* launches, uint64_t* particle_steps) {
+    if (!c) return AXG_EINVAL;
+    if (device_ms) *device_ms = c->last_ms;
+    if (launches) *launches = c->last_launches;
+    if (particle_steps) *particle_steps = c->last_particle_steps;
+    return AXG_OK;
+}
+
+AXG_API int axg_profile_next_step(axg_ctx* c, int enable) {
+    if (!c) return AXG_EINVAL;
+    c->profile_next = enable != 0;
+    return AXG_OK;
+}
+
+AXG_API int axg_kernel_times(axg_ctx* c, float* times_ms) {
+    if (!c || !times_ms) return AXG_EINVAL;
+    std::memcpy(times_ms, c->ktimes, sizeof(c->ktimes));
+    return AXG_OK;
+}

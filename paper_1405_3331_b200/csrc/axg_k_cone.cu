@@ -1,0 +1,213 @@
+// axg_k_cone.cu -- P3 sensing, P4 advance, P5 append (DESIGN.md §3 O7..O10).
+// Paper: neighbour-cell loop over the uniform grid, "vector addition" steering and "continue
+// on the current direction" when nothing is in range, a predefined distance per step
+// (PAPER.md:282), capsule appended at the end of the previous one, growth stops near a target or out of bounds
+// (PAPER.md:239), squared-distance test.
+#include "axg_dev.cuh"
+
+namespace {
+
+// ---- P3: one warp per cone; lanes take stencil cells; integer sums only (bit-exact) --------------------------
+// sense[c][s] = (n_s, Mx_s, My_s, Mz_s), M_s = sum over stencil offsets d of count_s(cell + d) * d   (reading A-12)
+__global__ void __launch_bounds__(256) k_sense(const AxgParams p) {
+    const int lane = threadIdx.x & 31;
+    const uint32_t warps_total = (gridDim.x * blockDim.x) >> 5;
+    const uint32_t* __restrict__ cell_lo = p.cell_lo;
+    for (uint32_t c = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; c < p.n_cones; c += warps_total) {
+        if (p.cone_state[c] != 0) continue;  // frozen cones skip P3..P5 (reading A-16)
+        const int ci = (int)p.cone_pos[c * 3 + 0], cj = (int)p.cone_pos[c * 3 + 1], ck = (int)p.cone_pos[c * 3 + 2];
+        int acc[AXG_MAX_SPECIES_D][4];
+#pragma unroll
+        for (int s = 0; s < AXG_MAX_SPECIES_D; ++s)
+#pragma unroll
+            for (int a = 0; a < 4; ++a) acc[s][a] = 0;
+        for (uint32_t e = lane; e < p.n_stencil; e += 32) {
+            const int32_t o = __ldg(p.stencil + e);
+            const int dx = (int)(int8_t)(o & 0xff), dy = (int)(int8_t)((o >> 8) & 0xff),
+                      dz = (int)(int8_t)((o >> 16) & 0xff);
+            const int x = ci + dx, y = cj + dy, z = ck + dz;
+            if (x < 0 || y < 0 || z < 0 || x >= (int)p.nx || y >= (int)p.ny || z >= (int)p.nz) continue;
+            const uint32_t cell = ((uint32_t)z * p.ny + (uint32_t)y) * p.nx + (uint32_t)x;
+            const uint32_t a = __ldg(cell_lo + cell), b = __ldg(cell_lo + cell + 1);
+            if (p.single_species >= 0) {
+                const int cnt = (int)(b - a);
+#pragma unroll
+                for (int s = 0; s < AXG_MAX_SPECIES_D; ++s)
+                    if (s == p.single_species) {
+                        acc[s][0] += cnt; acc[s][1] += cnt * dx; acc[s][2] += cnt * dy; acc[s][3] += cnt * dz;
+                    }
+            } else {
+                for (uint32_t j = a; j < b; ++j) {
+                    const int sp = (int)__ldg(p.A.species + j);
+#pragma unroll
+                    for (int s = 0; s < AXG_MAX_SPECIES_D; ++s)
+                        if (s == sp) { acc[s][0] += 1; acc[s][1] += dx; acc[s][2] += dy; acc[s][3] += dz; }
+                }
+            }
+        }
+        int mine = 0;
+        long long G[3] = {0, 0, 0};
+#pragma unroll
+        for (int s = 0; s < AXG_MAX_SPECIES_D; ++s)
+#pragma unroll
+            for (int a = 0; a < 4; ++a) {
+                const int v = __reduce_add_sync(0xffffffffu, acc[s][a]);
+                if (lane == s * 4 + a) mine = v;
+                if (a > 0) G[a - 1] += (long long)p.polarity[s] * v;
+            }
+        if (lane < 16) p.sense[(size_t)c * 16 + lane] = mine;
+        if (lane < 3) p.cone_gradient[c * 3 + lane] = (float)G[lane] / p.s2;  // g = G / S2(R)
+    }
+}
+
+// ---- P4 + P5: one thread per cone ------------------------------------------------------------------------------
+// Every fp32 operation that the specification fixes is written with the explicit round-to-nearest intrinsics so
+// that nvcc cannot contract it into an fma (reading A-22); only the normals may differ by an ulp.
+__global__ void __launch_bounds__(128) k_advance(const AxgParams p) {
+    AxgDev* dev = p.dev;
+    const uint32_t t = dev->step;
+    for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < p.n_cones; c += gridDim.x * blockDim.x) {
+        if (p.cone_state[c] != 0) continue;
+        long long G[3] = {0, 0, 0};
+#pragma unroll
+        for (int s = 0; s < AXG_MAX_SPECIES_D; ++s) {
+            const int4 v = *reinterpret_cast<const int4*>(p.sense + (size_t)c * 16 + s * 4);
+            G[0] += (long long)p.polarity[s] * v.y;
+            G[1] += (long long)p.polarity[s] * v.z;
+            G[2] += (long long)p.polarity[s] * v.w;
+        }
+        float h[3] = {p.cone_heading[c * 3 + 0], p.cone_heading[c * 3 + 1], p.cone_heading[c * 3 + 2]};
+        float q[3] = {p.cone_pos[c * 3 + 0], p.cone_pos[c * 3 + 1], p.cone_pos[c * 3 + 2]};
+        float g[3];
+        const float gx = (float)G[0], gy = (float)G[1], gz = (float)G[2];
+        p.cone_gradient[c * 3 + 0] = __fdiv_rn(gx, p.s2);  // rewritten here: with sharding the sums were
+        p.cone_gradient[c * 3 + 1] = __fdiv_rn(gy, p.s2);  // all-reduced after k_sense
+        p.cone_gradient[c * 3 + 2] = __fdiv_rn(gz, p.s2);
+        if (G[0] == 0 && G[1] == 0 && G[2] == 0) {  // reading A-14: keep the current direction
+            g[0] = h[0]; g[1] = h[1]; g[2] = h[2];
+        } else {
+            const float len = __fsqrt_rn(__fadd_rn(__fadd_rn(__fmul_rn(gx, gx), __fmul_rn(gy, gy)), __fmul_rn(gz, gz)));
+            g[0] = __fdiv_rn(gx, len); g[1] = __fdiv_rn(gy, len); g[2] = __fdiv_rn(gz, len);
+        }
+        float xi[3];
+        axg_normals3(c, t, 1u, p.seed_lo, p.seed_hi, xi[0], xi[1], xi[2]);  // stream 1 = cone noise (A-2)
+        float v[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) v[a] = __fadd_rn(g[a], __fmul_rn(p.noise, xi[a]));  // reading A-15
+        const float vlen =
+            __fsqrt_rn(__fadd_rn(__fadd_rn(__fmul_rn(v[0], v[0]), __fmul_rn(v[1], v[1])), __fmul_rn(v[2], v[2])));
+#pragma unroll
+        for (int a = 0; a < 3; ++a) h[a] = (vlen > 0.0f) ? __fdiv_rn(v[a], vlen) : g[a];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) q[a] = __fadd_rn(q[a], __fmul_rn(p.speed, h[a]));
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            p.cone_heading[c * 3 + a] = h[a];
+            p.cone_pos[c * 3 + a] = q[a];
+        }
+        // O9 append: step-major planes so that one step's appends of neighbouring cones coalesce
+        const uint32_t len = p.poly_len[c];
+        if (len <= p.max_segments) {
+#pragma unroll
+            for (int a = 0; a < 3; ++a) p.poly[((size_t)len * 3 + a) * p.n_cones + c] = q[a];
+            p.poly_len[c] = len + 1u;
+        } else {
+            atomicOr(&dev->err, 2u);
+        }
+        uint8_t state = 0;
+        if (!(q[0] >= 0.0f && q[0] < p.fnx && q[1] >= 0.0f && q[1] < p.fny && q[2] >= 0.0f && q[2] < p.fnz)) {
+            state = 2;  // exited
+        } else {
+            for (uint32_t s = 0; s < p.n_src; ++s) {  // reading A-16: targets = attractive sources, r_cap = 1
+                const AxgSourceDev sd = p.src[s];
+                if (!(sd.species_polarity & 0x100u)) continue;
+                const float dx = __fsub_rn(q[0], sd.x), dy = __fsub_rn(q[1], sd.y), dz = __fsub_rn(q[2], sd.z);
+                const float d2 = __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
+                if (d2 <= 1.0f) { state = 1; break; }
+            }
+        }
+        if (state) p.cone_state[c] = state;
+    }
+}
+
+__global__ void k_commit(const AxgParams p) { p.dev->step += 1u; }  // O10
+
+__global__ void k_census(const AxgParams p) {
+    __shared__ uint32_t s_c[4];
+    if (threadIdx.x < 4) s_c[threadIdx.x] = 0u;
+    __syncthreads();
+    for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < p.n_cones; c += gridDim.x * blockDim.x) {
+        const uint32_t st = p.cone_state[c];
+        if (st < 3u) atomicAdd(&s_c[st], 1u);
+        if (st == 0u) atomicMax(&s_c[3], p.poly_len[c]);  // longest ACTIVE polyline (capacity pre-check)
+    }
+    __syncthreads();
+    if (threadIdx.x < 3 && s_c[threadIdx.x]) atomicAdd(&p.dev->cone_census[threadIdx.x], s_c[threadIdx.x]);
+    if (threadIdx.x == 3) atomicMax(&p.dev->cone_census[3], s_c[3]);
+}
+
+// widen the int32 sensing sums to the ABI's int64 layouts
+__global__ void k_sense_export(const AxgParams p, long long* counts, long long* moment) {
+    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < p.n_cones * 4u; i += gridDim.x * blockDim.x) {
+        const int4 v = *reinterpret_cast<const int4*>(p.sense + (size_t)i * 4);
+        if (counts) counts[i] = v.x;
+        if (moment) { moment[(size_t)i * 3 + 0] = v.y; moment[(size_t)i * 3 + 1] = v.z; moment[(size_t)i * 3 + 2] = v.w; }
+    }
+}
+
+// step-major planes -> neuron-major AoS [C][max_segments+1][3]; entries >= poly_len are 0
+__global__ void k_poly_export(const AxgParams p, float* __restrict__ dst) {
+    const size_t rows = (size_t)p.max_segments + 1;
+    const size_t total = (size_t)p.n_cones * rows;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const uint32_t c = (uint32_t)(i / rows);
+        const size_t k = i % rows;
+        const bool live = k < p.poly_len[c];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) dst[i * 3 + a] = live ? p.poly[(k * 3 + a) * p.n_cones + c] : 0.0f;
+    }
+}
+
+// poly[len-1] = current position (axg_place_neurons / axg_load_cones)
+__global__ void k_poly_init(const AxgParams p) {
+    for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < p.n_cones; c += gridDim.x * blockDim.x) {
+        const uint32_t len = p.poly_len[c];
+        if (len >= 1u && len <= p.max_segments + 1u)
+            for (int a = 0; a < 3; ++a) p.poly[((size_t)(len - 1) * 3 + a) * p.n_cones + c] = p.cone_pos[c * 3 + a];
+    }
+}
+
+inline int grid_for(uint32_t n, int threads, int cap) {
+    long long g = ((long long)n + threads - 1) / threads;
+    if (g < 1) g = 1;
+    if (g > cap) g = cap;
+    return (int)g;
+}
+
+}  // namespace
+
+void axg_launch_sense(const AxgParams& p, cudaStream_t s) {
+    if (!p.n_cones) return;
+    k_sense<<<grid_for(p.n_cones, 8, 148 * 8), 256, 0, s>>>(p);
+}
+void axg_launch_advance(const AxgParams& p, cudaStream_t s) {
+    if (!p.n_cones) return;
+    k_advance<<<grid_for(p.n_cones, 128, 148 * 16), 128, 0, s>>>(p);
+}
+void axg_launch_commit(const AxgParams& p, cudaStream_t s) { k_commit<<<1, 1, 0, s>>>(p); }
+void axg_launch_census(const AxgParams& p, cudaStream_t s) {
+    if (!p.n_cones) return;
+    k_census<<<grid_for(p.n_cones, 256, 148 * 4), 256, 0, s>>>(p);
+}
+void axg_launch_sense_export(const AxgParams& p, long long* counts, long long* moment, cudaStream_t s) {
+    if (!p.n_cones) return;
+    k_sense_export<<<grid_for(p.n_cones * 4u, 256, 148 * 8), 256, 0, s>>>(p, counts, moment);
+}
+void axg_launch_poly_export(const AxgParams& p, float* dst, cudaStream_t s) {
+    if (!p.n_cones) return;
+    k_poly_export<<<148 * 8, 256, 0, s>>>(p, dst);
+}
+void axg_launch_poly_init(const AxgParams& p, cudaStream_t s) {
+    if (!p.n_cones) return;
+    k_poly_init<<<grid_for(p.n_cones, 256, 148 * 8), 256, 0, s>>>(p);
+}

@@ -1,0 +1,258 @@
+// axg_k_diffuse.cu -- P1 of the step (SURVEY.md §8(a) P1a..P1d + P2a; DESIGN.md §3 O1..O3):
+//   k_diffuse  Brownian step of every live particle (Philox4x32-10 keyed on (seed, id, t) -> Box-Muller -> fma),
+//              absorbing-boundary test, ORDER-PRESERVING compaction (warp ballot/popc ranks, block scan, one
+//              decoupled look-back word per tile), cell key, per-pass digit histograms for the radix sort.
+//   k_emit     newborns of every owned source appended after the survivors, counters, histogram scan.
+//   k_rekey    harness path (AXG_PHASE_BIN without AXG_PHASE_DIFFUSE): copy A -> B and key it.
+// Paper: integration kernel + calculateHash, PAPER.md:263 (§3.5); particles "generated ... and die".
+#include "axg_dev.cuh"
+
+namespace {
+
+constexpr int DIFF_THREADS = 256;
+constexpr int DIFF_ITEMS = 8;
+constexpr int DIFF_TILE = DIFF_THREADS * DIFF_ITEMS;
+constexpr int DIFF_WARPS = DIFF_THREADS / 32;
+
+__device__ __forceinline__ uint32_t cell_key(const AxgParams& p, float x, float y, float z) {
+    // O3 / reading A-8: truncation of non-negative fp32, x fastest
+    return ((uint32_t)z * p.ny + (uint32_t)y) * p.nx + (uint32_t)x;
+}
+
+__device__ __forceinline__ void hist_add(uint32_t (*s_hist)[AXG_RADIX], int n_pass, uint32_t key) {
+#pragma unroll
+    for (int q = 0; q < AXG_MAX_PASSES; ++q)
+        if (q < n_pass) atomicAdd(&s_hist[q][(key >> (8 * q)) & 0xffu], 1u);
+}
+
+__global__ void __launch_bounds__(DIFF_THREADS, 3) k_diffuse(const AxgParams p) {
+    __shared__ uint32_t s_hist[AXG_MAX_PASSES][AXG_RADIX];
+    __shared__ uint32_t s_warp[DIFF_WARPS];
+    __shared__ uint32_t s_tile, s_base;
+
+    AxgDev* dev = p.dev;
+    const uint32_t n_in = dev->n_live, t = dev->step, epoch = dev->epoch;
+    const uint32_t n_tiles = (n_in + DIFF_TILE - 1) / DIFF_TILE;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t lt = axg_lanemask_lt();
+
+    for (int i = tid; i < AXG_MAX_PASSES * AXG_RADIX; i += DIFF_THREADS) (&s_hist[0][0])[i] = 0u;
+
+    while (true) {
+        __syncthreads();  // s_tile / s_warp / s_base reuse, and s_hist zeroing on the first trip
+        if (tid == 0) s_tile = atomicAdd(&dev->ticket, 1u);
+        __syncthreads();
+        const uint32_t tile = s_tile;
+        if (tile >= n_tiles) break;
+
+        // ---- load: warp-striped, 128 B per warp request per column -------------------------------------
+        const uint32_t first = tile * DIFF_TILE + warp * (32 * DIFF_ITEMS) + lane;
+        float x[DIFF_ITEMS], y[DIFF_ITEMS], z[DIFF_ITEMS];
+        uint32_t id[DIFF_ITEMS];
+        uint32_t sp_pack[DIFF_ITEMS / 4];
+#pragma unroll
+        for (int k = 0; k < DIFF_ITEMS / 4; ++k) sp_pack[k] = 0u;
+#pragma unroll
+        for (int i = 0; i < DIFF_ITEMS; ++i) {
+            const uint32_t g = first + i * 32;
+            const bool v = g < n_in;
+            x[i] = v ? __ldg(p.A.x + g) : -1.0f;
+            y[i] = v ? __ldg(p.A.y + g) : -1.0f;
+            z[i] = v ? __ldg(p.A.z + g) : -1.0f;
+            id[i] = v ? __ldg(p.A.id + g) : 0u;
+            const uint32_t s = v ? (uint32_t)__ldg(p.A.species + g) : 0u;
+            sp_pack[i >> 2] |= s << (8 * (i & 3));
+        }
+
+        // ---- O1: diffuse; P1b: absorb ---------------------------------------------------------------------
+        uint32_t alive = 0u;
+#pragma unroll
+        for (int i = 0; i < DIFF_ITEMS; ++i) {
+            const bool v = (first + i * 32) < n_in;
+            float z0, z1, z2;
+            axg_normals3(id[i], t, 0u, p.seed_lo, p.seed_hi, z0, z1, z2);
+            x[i] = fmaf(p.sigma, z0, x[i]);
+            y[i] = fmaf(p.sigma, z1, y[i]);
+            z[i] = fmaf(p.sigma, z2, z[i]);
+            const bool in = x[i] >= 0.0f && x[i] < p.fnx && y[i] >= 0.0f && y[i] < p.fny && z[i] >= 0.0f &&
+                            z[i] < p.fnz;
+            alive |= (v && in) ? (1u << i) : 0u;
+        }
+
+        // ---- P1d: order-preserving ranks.  Order inside a warp chunk is (item, lane) = memory order. ---------
+        uint32_t wtotal = 0u;
+#pragma unroll
+        for (int i = 0; i < DIFF_ITEMS; ++i) wtotal += __popc(__ballot_sync(0xffffffffu, (alive >> i) & 1u));
+        if (lane == 0) s_warp[warp] = wtotal;
+        __syncthreads();
+        uint32_t woff = 0u, ttotal = 0u;
+#pragma unroll
+        for (int w = 0; w < DIFF_WARPS; ++w) {
+            const uint32_t c = s_warp[w];
+            woff += (w < warp) ? c : 0u;
+            ttotal += c;
+        }
+        if (warp == 0) {  // decoupled look-back, 32 predecessors per probe
+            uint32_t excl = 0u;
+            if (tile == 0) {
+                if (lane == 0) axg_st_state(p.tile_state + tile, axg_pack(epoch, AXG_FLAG_INCL, ttotal));
+            } else {
+                if (lane == 0) axg_st_state(p.tile_state + tile, axg_pack(epoch, AXG_FLAG_AGG, ttotal));
+                int q = (int)tile - 1 - lane;
+                while (true) {
+                    unsigned long long w;
+                    uint32_t f;
+                    do {
+                        w = (q >= 0) ? axg_ld_state(p.tile_state + q) : axg_pack(epoch, AXG_FLAG_INCL, 0u);
+                        f = axg_flag(w, epoch);
+                    } while (__any_sync(0xffffffffu, f == 0u));
+                    const uint32_t incl = __ballot_sync(0xffffffffu, f == (uint32_t)AXG_FLAG_INCL);
+                    uint32_t v = (uint32_t)w;
+                    if (incl) {
+                        const int firstincl = __ffs(incl) - 1;
+                        v = (lane <= firstincl) ? v : 0u;
+                        excl += __reduce_add_sync(0xffffffffu, v);
+                        break;
+                    }
+                    excl += __reduce_add_sync(0xffffffffu, v);
+                    q -= 32;
+                }
+                if (lane == 0) axg_st_state(p.tile_state + tile, axg_pack(epoch, AXG_FLAG_INCL, excl + ttotal));
+            }
+            if (lane == 0) {
+                s_base = excl;
+                if (tile == n_tiles - 1) dev->n_surv = excl + ttotal;
+            }
+        }
+        __syncthreads();
+        uint32_t out = s_base + woff;
+
+        // ---- write survivors (coalesced: consecutive lanes -> consecutive slots), key, histograms -------------
+#pragma unroll
+        for (int i = 0; i < DIFF_ITEMS; ++i) {
+            const uint32_t a = (alive >> i) & 1u;
+            const uint32_t b = __ballot_sync(0xffffffffu, a);
+            if (a) {
+                const uint32_t o = out + __popc(b & lt);
+                const uint32_t key = cell_key(p, x[i], y[i], z[i]);
+                p.B.x[o] = x[i];
+                p.B.y[o] = y[i];
+                p.B.z[o] = z[i];
+                p.B.id[o] = id[i];
+                p.B.species[o] = (uint8_t)((sp_pack[i >> 2] >> (8 * (i & 3))) & 0xffu);
+                p.key_pre[o] = key;
+                hist_add(s_hist, p.n_pass, key);
+            }
+            out += __popc(b);
+        }
+    }
+
+    __syncthreads();
+    for (int i = tid; i < p.n_pass * AXG_RADIX; i += DIFF_THREADS) {
+        const uint32_t c = (&s_hist[0][0])[i];
+        if (c) atomicAdd(&dev->hist[0][0] + i, c);
+    }
+    if (axg_last_block(dev) && tid == 0) {
+        dev->ticket = 0u;
+        dev->done = 0u;
+        dev->epoch = epoch + 1u;
+    }
+}
+
+// harness path: B = A, key_pre = key(A), histograms.  No RNG, no compaction.
+__global__ void __launch_bounds__(256) k_rekey(const AxgParams p) {
+    __shared__ uint32_t s_hist[AXG_MAX_PASSES][AXG_RADIX];
+    AxgDev* dev = p.dev;
+    const uint32_t n = dev->n_live;
+    for (int i = threadIdx.x; i < AXG_MAX_PASSES * AXG_RADIX; i += blockDim.x) (&s_hist[0][0])[i] = 0u;
+    __syncthreads();
+    for (uint32_t g = blockIdx.x * blockDim.x + threadIdx.x; g < n; g += gridDim.x * blockDim.x) {
+        const float x = p.A.x[g], y = p.A.y[g], z = p.A.z[g];
+        const uint32_t key = cell_key(p, x, y, z);
+        p.B.x[g] = x;
+        p.B.y[g] = y;
+        p.B.z[g] = z;
+        p.B.id[g] = p.A.id[g];
+        p.B.species[g] = p.A.species[g];
+        p.key_pre[g] = key;
+        hist_add(s_hist, p.n_pass, key);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < p.n_pass * AXG_RADIX; i += blockDim.x) {
+        const uint32_t c = (&s_hist[0][0])[i];
+        if (c) atomicAdd(&dev->hist[0][0] + i, c);
+    }
+}
+
+// O2: newborns (reading A-5: exactly at the source, not moved in their birth step; A-6: after the survivors, in
+// (source, j) order), counters, and the exclusive scans of the digit histograms that the sort passes start from.
+// One block.  do_emit == 0 is the harness path after k_rekey.
+constexpr int EMIT_THREADS = 1024;
+__global__ void __launch_bounds__(EMIT_THREADS) k_emit(const AxgParams p, int do_emit) {
+    __shared__ uint32_t s_hist[AXG_MAX_PASSES][AXG_RADIX];
+    __shared__ uint32_t s_scan[AXG_MAX_PASSES][AXG_RADIX / 32];
+    AxgDev* dev = p.dev;
+    const int tid = threadIdx.x;
+    const uint32_t n_in = dev->n_live;
+    const uint32_t n_surv = do_emit ? (n_in ? dev->n_surv : 0u) : n_in;
+    const uint32_t next_id = dev->next_id;
+    const bool fits = (unsigned long long)n_surv + p.e_owned <= (unsigned long long)p.capacity;
+    for (int i = tid; i < AXG_MAX_PASSES * AXG_RADIX; i += EMIT_THREADS) (&s_hist[0][0])[i] = 0u;
+    __syncthreads();
+    if (do_emit && fits) {
+        for (uint32_t e = tid; e < p.e_owned; e += EMIT_THREADS) {
+            // source s with src_emit_prefix[s] <= e < src_emit_prefix[s+1]
+            uint32_t lo = 0u, hi = p.n_src;
+            while (hi - lo > 1u) {
+                const uint32_t mid = (lo + hi) >> 1;
+                if (p.src_emit_prefix[mid] <= e) lo = mid; else hi = mid;
+            }
+            const uint32_t s = lo, j = e - p.src_emit_prefix[s];
+            const AxgSourceDev sd = p.src[s];
+            const uint32_t o = n_surv + e;
+            const uint32_t key = cell_key(p, sd.x, sd.y, sd.z);
+            p.B.x[o] = sd.x;
+            p.B.y[o] = sd.y;
+            p.B.z[o] = sd.z;
+            p.B.species[o] = (uint8_t)(sd.species_polarity & 0xffu);
+            p.B.id[o] = next_id + p.src_id_prefix[s] + j;
+            p.key_pre[o] = key;
+            hist_add(s_hist, p.n_pass, key);
+        }
+    }
+    __syncthreads();
+    // total histogram -> exclusive scan per pass (1024 threads = 4 passes x 256 digits)
+    const int q = tid >> 8, d = tid & 255, lane = tid & 31, wq = d >> 5;
+    uint32_t c = 0u;
+    if (q < p.n_pass) c = dev->hist[q][d] + s_hist[q][d];
+    uint32_t inc = c;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += v;
+    }
+    if (lane == 31) s_scan[q][wq] = inc;
+    __syncthreads();
+    uint32_t off = 0u;
+    for (int w = 0; w < wq; ++w) off += s_scan[q][w];
+    dev->base[q][d] = off + inc - c;
+    dev->hist[q][d] = 0u;
+    if (tid == 0) {
+        if (do_emit) {
+            if (!fits) dev->err |= 1u;
+            dev->n_live = fits ? n_surv + p.e_owned : n_surv;
+            dev->next_id = next_id + p.e_total;
+            dev->emitted += fits ? p.e_owned : 0u;
+            dev->absorbed += n_in - n_surv;
+            dev->particle_steps += n_in;
+        }
+    }
+}
+
+}  // namespace
+
+int axg_diffuse_tile() { return DIFF_TILE; }
+
+void axg_launch_diffuse(const AxgParams& p, int grid, cudaStream_t s) { k_diffuse<<<grid, DIFF_THREADS, 0, s>>>(p); }
+void axg_launch_rekey(const AxgParams& p, int grid, cudaStream_t s) { k_rekey<<<grid, 256, 0, s>>>(p); }
+void axg_launch_emit(const AxgParams& p, int do_emit, cudaStream_t s) { k_emit<<<1, EMIT_THREADS, 0, s>>>(p, do_emit); }

@@ -1,0 +1,160 @@
+// axg_k_sort.cu -- P2b: stable LSD radix sort of (key, pre-sort index), 8-bit digits, one kernel per digit pass
+// (DESIGN.md §3 O4, reading A-9).  The paper sorts (cell hash, particle id) pairs with a
+// library radix sort; this is a hand-written single-pass-per-digit ("onesweep"-style) sort:
+//   - digit histograms of ALL passes are known before the first pass (accumulated by k_diffuse / k_emit),
+//   - inside a tile every warp ranks its keys in memory order with __match_any_sync + popc (stable),
+//   - per-tile per-digit counts chain across tiles by decoupled look-back (one 64-bit word per tile and digit,
+//     epoch-tagged so the words never need clearing),
+//   - the tile is sorted through shared memory so that global stores run along digit runs.
+#include "axg_dev.cuh"
+
+namespace {
+
+constexpr int SORT_THREADS = 512;
+constexpr int SORT_ITEMS = 12;
+constexpr int SORT_WARPS = SORT_THREADS / 32;
+constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;
+constexpr size_t SORT_SMEM = (size_t)(2 * SORT_TILE + SORT_WARPS * AXG_RADIX + 2 * AXG_RADIX + 16) * sizeof(uint32_t);
+
+template <bool FIRST>
+__global__ void __launch_bounds__(SORT_THREADS, 2)
+k_sort_pass(const AxgParams p, const int pass, const uint32_t* __restrict__ kin, const uint32_t* __restrict__ vin,
+            uint32_t* __restrict__ kout, uint32_t* __restrict__ vout) {
+    extern __shared__ uint32_t smem[];
+    uint32_t* s_key = smem;
+    uint32_t* s_val = s_key + SORT_TILE;
+    uint32_t* s_wh = s_val + SORT_TILE;                 // [SORT_WARPS][256] per-warp digit counts -> offsets
+    uint32_t* s_dstart = s_wh + SORT_WARPS * AXG_RADIX; // [256] first tile-local slot of the digit
+    uint32_t* s_gbase = s_dstart + AXG_RADIX;           // [256] global slot of tile-local slot 0 of the digit run
+    uint32_t* s_misc = s_gbase + AXG_RADIX;             // [0] tile ticket, [1..8] warp scan partials
+
+    AxgDev* dev = p.dev;
+    const uint32_t n = dev->n_live, epoch = dev->epoch;
+    const uint32_t n_tiles = (n + SORT_TILE - 1) / SORT_TILE;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t lt = axg_lanemask_lt();
+    const int shift = 8 * pass;
+    uint32_t* my_wh = s_wh + warp * AXG_RADIX;
+
+    while (true) {
+        __syncthreads();
+        if (tid == 0) s_misc[0] = atomicAdd(&dev->ticket, 1u);
+#pragma unroll
+        for (int i = 0; i < AXG_RADIX / 32; ++i) my_wh[i * 32 + lane] = 0u;
+        __syncthreads();
+        const uint32_t tile = s_misc[0];
+        if (tile >= n_tiles) break;
+
+        const uint32_t first = tile * SORT_TILE + warp * (32 * SORT_ITEMS) + lane;
+        uint32_t key[SORT_ITEMS], val[SORT_ITEMS], rank[SORT_ITEMS];
+#pragma unroll
+        for (int i = 0; i < SORT_ITEMS; ++i) {
+            const uint32_t g = first + i * 32;
+            key[i] = (g < n) ? __ldg(kin + g) : 0xffffffffu;
+            val[i] = FIRST ? g : ((g < n) ? __ldg(vin + g) : 0u);
+        }
+        // ---- rank inside the warp chunk, in memory order (item, lane) ------------------------------------
+#pragma unroll
+        for (int i = 0; i < SORT_ITEMS; ++i) {
+            const uint32_t d = (key[i] >> shift) & 0xffu;
+            const uint32_t m = __match_any_sync(0xffffffffu, d);
+            const int leader = __ffs(m) - 1;
+            uint32_t old = 0u;
+            if (lane == leader) {
+                old = my_wh[d];
+                my_wh[d] = old + __popc(m);
+            }
+            __syncwarp();
+            old = __shfl_sync(0xffffffffu, old, leader);
+            rank[i] = old + __popc(m & lt);
+        }
+        __syncthreads();
+        // ---- per digit: scan over warps, scan over digits, look-back over tiles ----------------------------
+        if (tid < AXG_RADIX) {
+            const int d = tid;
+            uint32_t run = 0u;
+#pragma unroll
+            for (int w = 0; w < SORT_WARPS; ++w) {
+                const uint32_t c = s_wh[w * AXG_RADIX + d];
+                s_wh[w * AXG_RADIX + d] = run;
+                run += c;
+            }
+            const uint32_t count = run;
+            unsigned long long* st = p.sort_state + (size_t)tile * AXG_RADIX + d;
+            axg_st_state(st, axg_pack(epoch, tile == 0 ? AXG_FLAG_INCL : AXG_FLAG_AGG, count));
+            uint32_t inc = count;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o);
+                if (lane >= o) inc += v;
+            }
+            if (lane == 31) s_misc[1 + warp] = inc;
+            asm volatile("bar.sync 1, 256;");  // the 8 warps that own the digits
+            uint32_t off = 0u;
+            for (int w = 0; w < warp; ++w) off += s_misc[1 + w];
+            const uint32_t dstart = off + inc - count;
+            s_dstart[d] = dstart;
+            uint32_t excl = 0u;
+            if (tile > 0) {
+                for (int q = (int)tile - 1;; --q) {
+                    unsigned long long w;
+                    uint32_t f;
+                    do {
+                        w = axg_ld_state(p.sort_state + (size_t)q * AXG_RADIX + d);
+                        f = axg_flag(w, epoch);
+                    } while (f == 0u);
+                    excl += (uint32_t)w;
+                    if (f == (uint32_t)AXG_FLAG_INCL) break;
+                }
+                axg_st_state(st, axg_pack(epoch, AXG_FLAG_INCL, excl + count));
+            }
+            s_gbase[d] = dev->base[pass][d] + excl - dstart;
+        }
+        __syncthreads();
+        // ---- sort the tile through shared memory ----------------------------------------------------------
+#pragma unroll
+        for (int i = 0; i < SORT_ITEMS; ++i) {
+            const uint32_t d = (key[i] >> shift) & 0xffu;
+            const uint32_t pos = s_dstart[d] + my_wh[d] + rank[i];
+            s_key[pos] = key[i];
+            s_val[pos] = val[i];
+        }
+        __syncthreads();
+        const uint32_t tile_n = min((uint32_t)SORT_TILE, n - tile * SORT_TILE);
+#pragma unroll
+        for (int i = 0; i < SORT_ITEMS; ++i) {
+            const uint32_t pos = tid + i * SORT_THREADS;
+            if (pos < tile_n) {
+                const uint32_t k = s_key[pos];
+                const uint32_t g = s_gbase[(k >> shift) & 0xffu] + pos;
+                kout[g] = k;
+                vout[g] = s_val[pos];
+            }
+        }
+    }
+    if (axg_last_block(dev) && tid == 0) {
+        dev->ticket = 0u;
+        dev->done = 0u;
+        dev->epoch = epoch + 1u;
+    }
+}
+
+}  // namespace
+
+int axg_sort_tile() { return SORT_TILE; }
+
+void axg_launch_sort_pass(const AxgParams& p, int pass, int grid, cudaStream_t s) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(k_sort_pass<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SORT_SMEM);
+        cudaFuncSetAttribute(k_sort_pass<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SORT_SMEM);
+        attr_set = true;
+    }
+    if (pass == 0) {
+        k_sort_pass<true><<<grid, SORT_THREADS, SORT_SMEM, s>>>(p, 0, p.key_pre, nullptr, p.skey[0], p.sidx[0]);
+    } else {
+        const int in = (pass - 1) & 1, out = pass & 1;
+        k_sort_pass<false><<<grid, SORT_THREADS, SORT_SMEM, s>>>(p, pass, p.skey[in], p.sidx[in], p.skey[out],
+                                                                  p.sidx[out]);
+    }
+}
