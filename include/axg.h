@@ -158,12 +158,27 @@ int axg_load_cones(axg_ctx* ctx, const float* pos, const float* heading, const u
 int axg_step_phase(axg_ctx* ctx, uint32_t phase_mask);
 
 /* Multi-GPU sharding by source: this rank emits only sources with index % world == rank; the
- * others still consume their particle ids, so trajectories equal the 1-GPU run.  Default (0,1).           */
+ * others still consume their particle ids, so trajectories equal the 1-GPU run.  Default (0,1).  With world > 1
+ * P3 writes zeros for frozen cones (so that the all-reduced buffer stays meaningful); their AXG_CONE_COUNTS /
+ * AXG_CONE_MOMENT then read 0 instead of the last active value.                                           */
 int axg_set_shard(axg_ctx* ctx, uint32_t rank, uint32_t world);
 
 /* Device pointer (int32[C][AXG_MAX_SPECIES][4] = n,Mx,My,Mz) of the per-cone sensing sums, for the NCCL
  * all-reduce between P3 and P4 when sharded.  *bytes = its size.  Owned by ctx.                           */
 int axg_sense_buffer(axg_ctx* ctx, void** device_ptr, size_t* bytes);
+
+/* The sharded step loop without a host synchronisation per step:
+ *     axg_check_capacity(ctx, n);
+ *     n times { axg_enqueue_phase(ctx, DIFFUSE|BIN|SENSE);  all-reduce of axg_sense_buffer on the ctx stream;
+ *               axg_enqueue_phase(ctx, ADVANCE|COMMIT); }
+ *     axg_sync(ctx);
+ * axg_check_capacity is the host-side pre-check that axg_step does for n further steps (AXG_ECAPACITY, nothing
+ * changed).  axg_enqueue_phase launches the kernels of the selected phases of ONE step on the ctx stream and returns
+ * at once; it checks nothing.  axg_sync waits for the stream, reads the device error word (AXG_ECAPACITY if set,
+ * AXG_ECUDA on a CUDA error) and refreshes the element counts that axg_read_state reports.                */
+int axg_check_capacity(axg_ctx* ctx, uint32_t n);
+int axg_enqueue_phase(axg_ctx* ctx, uint32_t phase_mask);
+int axg_sync(axg_ctx* ctx);
 
 /* Use `stream` (a cudaStream_t) for all later work of this ctx.                                          */
 int axg_set_stream(axg_ctx* ctx, void* stream);

@@ -54,6 +54,7 @@ def lib():
         L.axo_load_particles.argtypes = [vp, vp, vp, vp, vp, vp, u64, u32, u32]
         L.axo_load_cones.argtypes = [vp, vp, vp, vp, vp, u32]
         L.axo_read_state.argtypes = [vp, u32, vp, C.c_size_t, C.POINTER(C.c_size_t)]
+        L.axo_load_sense.argtypes = [vp, vp, vp, u32]
         L.axo_philox4x32_10.argtypes = [vp, vp, vp]
         L.axo_philox4x32_10.restype = None
         L.axo_normals.argtypes = [u64, u32, u32, u32, u32, vp, vp, vp]
@@ -134,6 +135,21 @@ class Oracle:
         state = np.ascontiguousarray(state, dtype=np.uint8)
         poly_len = np.ascontiguousarray(poly_len, dtype=np.uint32)
         self._chk(self._L.axo_load_cones(self._h, _ptr(pos), _ptr(heading), _ptr(state), _ptr(poly_len), pos.shape[0]))
+
+    # the sharded loop's call names (paper_1405_3331_b200/sharded.py drives either binding)
+    def check_capacity(self, n):
+        pass
+
+    def enqueue_phase(self, mask):
+        self.step_phase(mask)
+
+    def sync(self):
+        pass
+
+    def load_sense(self, counts, moment):
+        counts = np.ascontiguousarray(counts, dtype=np.int64)
+        moment = np.ascontiguousarray(moment, dtype=np.int64)
+        self._chk(self._L.axo_load_sense(self._h, _ptr(counts), _ptr(moment), counts.size // 4))
 
     def read_state(self, field):
         f = FIELDS[field] if isinstance(field, str) else int(field)

@@ -562,6 +562,16 @@ AXO_API int axo_read_state(axo_ctx* c, uint32_t field, void* dst, size_t dst_byt
     }
 }
 
+// Harness-only load hook for the sharded loop (world_size-2 gloo tests): replace the per-cone sums of the last P3
+// (e.g. by their sum over ranks) before P4 reads them.  No arithmetic: P4 recomputes G from these.
+AXO_API int axo_load_sense(axo_ctx* c, const int64_t* counts, const int64_t* moment, uint32_t n) {
+    if (!c || !counts || !moment) return fail(c, EINVAL_, "null argument");
+    if (n != c->n_cones()) return fail(c, EINVAL_, "cone count differs from the placed count");
+    c->cone_counts.assign(counts, counts + (size_t)n * MAX_SPECIES);
+    c->cone_moment.assign(moment, moment + (size_t)n * MAX_SPECIES * 3);
+    return OK;
+}
+
 // ---- oracle-only entry points used by the pins --------------------------------------------------------------
 
 // T1: the raw block function.

@@ -31,7 +31,7 @@ EXPORTS = (
     "axg_create", "axg_place_neurons", "axg_add_source", "axg_step", "axg_read_state", "axg_destroy",
     "axg_last_error", "axg_set_capacity", "axg_load_particles", "axg_load_cones", "axg_step_phase", "axg_set_shard",
     "axg_sense_buffer", "axg_set_stream", "axg_set_allocator", "axg_last_step_stats", "axg_profile_next_step",
-    "axg_kernel_times",
+    "axg_kernel_times", "axg_check_capacity", "axg_enqueue_phase", "axg_sync",
 )
 
 _ALLOC_T = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p)
@@ -78,6 +78,9 @@ def lib(build=True):
     L.axg_set_shard.argtypes = [vp, u32, u32]
     L.axg_step.argtypes = [vp, u32]
     L.axg_step_phase.argtypes = [vp, u32]
+    L.axg_check_capacity.argtypes = [vp, u32]
+    L.axg_enqueue_phase.argtypes = [vp, u32]
+    L.axg_sync.argtypes = [vp]
     L.axg_load_particles.argtypes = [vp, vp, vp, vp, vp, vp, u64, u32, u32]
     L.axg_load_cones.argtypes = [vp, vp, vp, vp, vp, u32]
     L.axg_read_state.argtypes = [vp, u32, vp, sz, C.POINTER(sz)]
@@ -179,6 +182,15 @@ class Axg:
 
     def step_phase(self, mask):
         self._chk(self._L.axg_step_phase(self._h, mask))
+
+    def check_capacity(self, n):
+        self._chk(self._L.axg_check_capacity(self._h, n))
+
+    def enqueue_phase(self, mask):
+        self._chk(self._L.axg_enqueue_phase(self._h, mask))
+
+    def sync(self):
+        self._chk(self._L.axg_sync(self._h))
 
     def load_particles(self, x, y, z, species, ids, next_id, step):
         x = np.ascontiguousarray(x, dtype=np.float32)

@@ -64,7 +64,7 @@ struct axg_ctx {
     // stats of the last axg_step
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     float last_ms = 0.f;
-    uint64_t last_launches = 0, last_particle_steps = 0;
+    uint64_t last_launches = 0, last_particle_steps = 0, ps0 = 0;
     bool profile_next = false;
     float ktimes[AXG_KERNEL_COUNT] = {0};
     std::vector<cudaEvent_t> prof_events;
@@ -451,6 +451,7 @@ AXG_API int axg_set_stream(axg_ctx* c, void* stream) {
 AXG_API int axg_set_shard(axg_ctx* c, uint32_t rank, uint32_t world) {
     if (!c || world == 0 || rank >= world) return fail(c, AXG_EINVAL, "bad shard");
     c->shard_rank = rank; c->shard_world = world;
+    c->P.sharded = world > 1 ? 1 : 0;
     return upload_sources(c);
 }
 
@@ -623,6 +624,42 @@ AXG_API int axg_step(axg_ctx* c, uint32_t n) {
         std::snprintf(msg, sizeof msg, "device error word 0x%x (1 = particle capacity, 2 = polyline capacity)", h.err);
         return fail(c, AXG_ECAPACITY, msg);
     }
+    return AXG_OK;
+}
+
+AXG_API int axg_check_capacity(axg_ctx* c, uint32_t n) {
+    if (!c) return AXG_EINVAL;
+    int rc = ensure_particles(c);
+    if (rc) return rc;
+    AxgDev h;
+    rc = capacity_check(c, n, true, true, &h);
+    if (rc) return rc;
+    c->last_launches = 0;            // the enqueue loop that follows is accounted like one axg_step call
+    c->ps0 = h.particle_steps;
+    return AXG_OK;
+}
+
+AXG_API int axg_enqueue_phase(axg_ctx* c, uint32_t mask) {
+    if (!c || (mask & ~(uint32_t)AXG_PHASE_ALL)) return fail(c, AXG_EINVAL, "bad phase mask");
+    int rc = ensure_particles(c);
+    if (rc) return rc;
+    Prof prof{c, false};
+    c->last_launches += (uint64_t)enqueue_phases(c, mask, prof);
+    c->stepped = true;
+    return AXG_OK;
+}
+
+AXG_API int axg_sync(axg_ctx* c) {
+    if (!c) return AXG_EINVAL;
+    int rc = after_sync(c, "axg_sync");
+    if (rc) return rc;
+    if (!c->d_dev) return AXG_OK;
+    AxgDev h;
+    rc = read_dev(c, &h);
+    if (rc) return rc;
+    c->n_A = c->n_B = h.n_live;
+    c->last_particle_steps = h.particle_steps - c->ps0;
+    if (h.err) return fail(c, AXG_ECAPACITY, "device error word set");
     return AXG_OK;
 }
 

@@ -14,7 +14,10 @@ __global__ void __launch_bounds__(256) k_sense(const AxgParams p) {
     const uint32_t warps_total = (gridDim.x * blockDim.x) >> 5;
     const uint32_t* __restrict__ cell_lo = p.cell_lo;
     for (uint32_t c = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; c < p.n_cones; c += warps_total) {
-        if (p.cone_state[c] != 0) continue;  // frozen cones skip P3..P5 (reading A-16)
+        if (p.cone_state[c] != 0) {  // frozen cones skip P3..P5 (reading A-16)
+            if (p.sharded && lane < 16) p.sense[(size_t)c * 16 + lane] = 0;
+            continue;
+        }
         const int ci = (int)p.cone_pos[c * 3 + 0], cj = (int)p.cone_pos[c * 3 + 1], ck = (int)p.cone_pos[c * 3 + 2];
         int acc[AXG_MAX_SPECIES_D][4];
 #pragma unroll

@@ -168,3 +168,80 @@ def apply(sim, w: Workload, place=True):
     if place and len(w.neurons):
         sim.place_neurons(w.neurons, None)
     return sim
+
+
+def synthetic_population(w: Workload, n, seed):
+    """n particle rows shaped like the steady state of `w` WITHOUT running the method (input for CPU timing samples,
+    bench.py `cpu_baseline` / `--impl reference`): per source a cloud whose width is drawn log-uniformly between one
+    cell and the box size (dense within a few cells of the source, ~uniform far away), clipped by rejection to the
+    box.  Species = the source's.  Ids 0..n-1 in a seeded random order."""
+    rng = np.random.default_rng(seed)
+    nx, ny, nz = w.grid
+    src = np.array([[s[0], s[1], s[2]] for s in w.sources], dtype=np.float64)
+    sp_of = np.array([s[3] for s in w.sources], dtype=np.uint8)
+    out_p, out_s = [], []
+    need = n
+    while need > 0:
+        m = int(need * 1.6) + 64
+        which = rng.integers(0, len(src), m)
+        width = np.exp(rng.uniform(0.0, np.log(max(nx, ny, nz) / 2.0), m))
+        p = src[which] + rng.normal(0.0, 1.0, (m, 3)) * width[:, None]
+        ok = (p[:, 0] >= 0) & (p[:, 0] < nx - 1e-3) & (p[:, 1] >= 0) & (p[:, 1] < ny - 1e-3) & (p[:, 2] >= 0) & \
+             (p[:, 2] < nz - 1e-3)
+        p, s = p[ok][:need], sp_of[which[ok]][:need]
+        out_p.append(p.astype(np.float32))
+        out_s.append(s)
+        need -= len(p)
+    p = np.concatenate(out_p, 0)
+    species = np.concatenate(out_s, 0)
+    ids = rng.permutation(n).astype(np.uint32)
+    return p[:, 0].copy(), p[:, 1].copy(), p[:, 2].copy(), species, ids
+
+
+def prerun(make_sim, w: Workload, coarse=16, relax=100, progress=None):
+    """Bring a fresh simulation of `w` to its steady state with the library itself (DESIGN.md §4 "reaching the
+    steady state"): a second context WITHOUT cones runs prerun_steps/coarse steps with D' = coarse*D and
+    rate' = coarse*rate (the continuous steady state depends on rate/D only), its particle array is handed to the
+    real context through read_state -> load_particles, and `relax` real steps wash out the coarse wall layer.
+    `make_sim(D, emission)` returns an object with the boundary's call names.  coarse <= 1: plain pre-run.
+    Returns the simulation, with neurons placed and the step counter at 0."""
+    if w.prerun_steps <= 0:
+        return apply(make_sim(w.D, w.emission), w)
+    if coarse <= 1:
+        pre = apply(make_sim(w.D, w.emission), w, place=False)
+        pre.step(w.prerun_steps)
+        cols = [pre.read_state("PART_" + k).copy() for k in ("X", "Y", "Z", "SPECIES", "ID")]
+        next_id = pre.counters()["next_id"]
+        pre.close()
+        relax = 0
+    else:
+        pre = make_sim(w.D * coarse, w.emission * coarse)
+        pre.set_capacity(w.max_particles or (1 << 20), 1)
+        for s in w.sources:
+            pre.add_source(s[0], s[1], s[2], s[3], s[4], s[5] * coarse)
+        cap = w.max_particles or (1 << 20)
+        e_coarse = sum(s[5] for s in w.sources) * coarse
+        todo = max(1, w.prerun_steps // coarse)
+        while todo > 0:
+            # the boundary refuses a call whose host-side bound n_live + k * E could overflow the capacity
+            n_live = pre.counters()["n_live"]
+            k = int(min(todo, 256, max(1, (cap - n_live) // max(e_coarse, 1))))
+            pre.step(k)
+            todo -= k
+            if progress:
+                progress(n_live)
+        cols = [pre.read_state("PART_" + k).copy() for k in ("X", "Y", "Z", "SPECIES", "ID")]
+        next_id = pre.counters()["next_id"]
+        pre.close()
+    if relax:                # a cone-less context with the real D washes out the coarse wall layer
+        mid = make_sim(w.D, w.emission)
+        apply(mid, w, place=False)
+        mid.load_particles(*cols, next_id=next_id, step=0)
+        mid.step(relax)
+        cols = [mid.read_state("PART_" + k).copy() for k in ("X", "Y", "Z", "SPECIES", "ID")]
+        next_id = mid.counters()["next_id"]
+        mid.close()
+    sim = make_sim(w.D, w.emission)
+    apply(sim, w)            # neurons are placed before the first step (AXG_ESTATE afterwards)
+    sim.load_particles(*cols, next_id=next_id, step=0)
+    return sim
