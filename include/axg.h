@@ -139,7 +139,8 @@ const char* axg_last_error(const axg_ctx* ctx);
 /* ---- harness / plumbing calls (not part of the paper's problem statement) ------------------------------- */
 
 /* Re-allocate for at most max_particles live particles and max_segments appended segments per cone.
- * Keeps sources and neurons; live particles are kept if they fit, else AXG_ECAPACITY.                     */
+ * Keeps sources and neurons; live particles are kept if they fit, else AXG_ECAPACITY.  max_particles < 2^30 - 256
+ * (the sort value carries the species in its top two bits), else AXG_EINVAL.                              */
 int axg_set_capacity(axg_ctx* ctx, uint64_t max_particles, uint32_t max_segments);
 
 /* Replace the particle array (taken as the "sorted order" array, i.e. the input of the next P1) and the id /

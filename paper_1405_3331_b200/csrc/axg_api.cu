@@ -182,12 +182,13 @@ int alloc_particles(axg_ctx* c, uint64_t cap, AxgParams& P, std::vector<void*>& 
     const size_t pad = 64;  // tail padding so that ragged tiles may over-read harmlessly
     const size_t n = (size_t)cap + pad;
     const size_t diff_tiles = n / axg_diffuse_tile() + 2, sort_tiles = n / axg_sort_tile() + 2;
-    const size_t sizes[] = {n * 4, n * 4, n * 4, n, n * 4,  // A
-                            n * 4, n * 4, n * 4, n, n * 4,  // B
+    const size_t sizes[] = {n * 4, n * 4, n * 4, n, n * 4,  // A (SoA)
+                            n * 16, n,                      // Brec, Bsp
                             n * 4, n * 4, n * 4, n * 4, n * 4,  // key_pre, skey[2], sidx[2]
                             diff_tiles * 8, sort_tiles * AXG_RADIX * 8};
-    void* ptr[17];
-    for (int i = 0; i < 17; ++i) {
+    constexpr int NB = 14;
+    void* ptr[NB];
+    for (int i = 0; i < NB; ++i) {
         ptr[i] = dev_alloc(c, sizes[i]);
         if (!ptr[i]) {
             for (int k = 0; k < i; ++k) dev_free(ptr[k]);
@@ -197,16 +198,17 @@ int alloc_particles(axg_ctx* c, uint64_t cap, AxgParams& P, std::vector<void*>& 
         bufs.push_back(ptr[i]);
     }
     P.A = AxgSoA{(float*)ptr[0], (float*)ptr[1], (float*)ptr[2], (uint8_t*)ptr[3], (uint32_t*)ptr[4]};
-    P.B = AxgSoA{(float*)ptr[5], (float*)ptr[6], (float*)ptr[7], (uint8_t*)ptr[8], (uint32_t*)ptr[9]};
-    P.key_pre = (uint32_t*)ptr[10];
-    P.skey[0] = (uint32_t*)ptr[11]; P.skey[1] = (uint32_t*)ptr[12];
-    P.sidx[0] = (uint32_t*)ptr[13]; P.sidx[1] = (uint32_t*)ptr[14];
-    P.tile_state = (unsigned long long*)ptr[15];
-    P.sort_state = (unsigned long long*)ptr[16];
+    P.Brec = (float4*)ptr[5];
+    P.Bsp = (uint8_t*)ptr[6];
+    P.key_pre = (uint32_t*)ptr[7];
+    P.skey[0] = (uint32_t*)ptr[8]; P.skey[1] = (uint32_t*)ptr[9];
+    P.sidx[0] = (uint32_t*)ptr[10]; P.sidx[1] = (uint32_t*)ptr[11];
+    P.tile_state = (unsigned long long*)ptr[12];
+    P.sort_state = (unsigned long long*)ptr[13];
     P.capacity = (uint32_t)cap;
     // look-back words must not alias a live epoch: zero them (epoch 0 words with flag 0 = not ready)
-    CU(c, cudaMemsetAsync(ptr[15], 0, sizes[15], c->stream));
-    CU(c, cudaMemsetAsync(ptr[16], 0, sizes[16], c->stream));
+    CU(c, cudaMemsetAsync(ptr[12], 0, sizes[12], c->stream));
+    CU(c, cudaMemsetAsync(ptr[13], 0, sizes[13], c->stream));
     return AXG_OK;
 }
 
@@ -497,7 +499,7 @@ AXG_API int axg_place_neurons(axg_ctx* c, const float* xyz, const float* heading
 }
 
 AXG_API int axg_set_capacity(axg_ctx* c, uint64_t max_particles, uint32_t max_segments) {
-    if (!c || max_particles == 0 || max_particles >= 0xffffff00ull) return fail(c, AXG_EINVAL, "bad capacity");
+    if (!c || max_particles == 0 || max_particles >= 0x3fffff00ull) return fail(c, AXG_EINVAL, "bad capacity");
     int rc = alloc_fixed(c);
     if (rc) return rc;
     AxgDev h;
@@ -745,7 +747,9 @@ AXG_API int axg_read_state(axg_ctx* c, uint32_t field, void* dst, size_t dst_byt
         case AXG_PART_SPECIES: return copy_out(c, P.A.species, nA, 1, dst, dst_bytes, n_elems);
         case AXG_PART_ID: return copy_out(c, P.A.id, nA, 4, dst, dst_bytes, n_elems);
         case AXG_KEYS_SORTED: return copy_out(c, have_p ? P.skey[P.final_buf] : nullptr, nB, 4, dst, dst_bytes, n_elems);
-        case AXG_PERM: return copy_out(c, have_p ? P.sidx[P.final_buf] : nullptr, nB, 4, dst, dst_bytes, n_elems);
+        case AXG_PERM:
+            return export_out(c, nB, 4, dst, dst_bytes, n_elems,
+                              [&](void* t) { axg_launch_perm_export(P, (uint32_t*)t, c->stream); });
         case AXG_CELL_START:
             return export_out(c, c->cells(), 4, dst, dst_bytes, n_elems,
                               [&](void* t) { axg_launch_cell_export(P, (uint32_t*)t, nullptr, c->stream); });
@@ -766,11 +770,15 @@ AXG_API int axg_read_state(axg_ctx* c, uint32_t field, void* dst, size_t dst_byt
         case AXG_POLYLINE:
             return export_out(c, C * ((size_t)c->max_segments + 1) * 3, 4, dst, dst_bytes, n_elems,
                               [&](void* t) { axg_launch_poly_export(P, (float*)t, c->stream); });
-        case AXG_PRE_X: return copy_out(c, P.B.x, nB, 4, dst, dst_bytes, n_elems);
-        case AXG_PRE_Y: return copy_out(c, P.B.y, nB, 4, dst, dst_bytes, n_elems);
-        case AXG_PRE_Z: return copy_out(c, P.B.z, nB, 4, dst, dst_bytes, n_elems);
-        case AXG_PRE_SPECIES: return copy_out(c, P.B.species, nB, 1, dst, dst_bytes, n_elems);
-        case AXG_PRE_ID: return copy_out(c, P.B.id, nB, 4, dst, dst_bytes, n_elems);
+        case AXG_PRE_X:
+        case AXG_PRE_Y:
+        case AXG_PRE_Z:
+        case AXG_PRE_ID: {
+            const int comp = field == AXG_PRE_ID ? 3 : (int)(field - AXG_PRE_X);
+            return export_out(c, nB, 4, dst, dst_bytes, n_elems,
+                              [&](void* t) { axg_launch_pre_export(P, comp, (uint32_t*)t, c->stream); });
+        }
+        case AXG_PRE_SPECIES: return copy_out(c, P.Bsp, nB, 1, dst, dst_bytes, n_elems);
         case AXG_PRE_KEY: return copy_out(c, P.key_pre, nB, 4, dst, dst_bytes, n_elems);
         default: return fail(c, AXG_EINVAL, "unknown field");
     }

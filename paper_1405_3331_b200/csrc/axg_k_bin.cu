@@ -10,59 +10,112 @@
 namespace {
 
 constexpr int BIN_THREADS = 256;
-constexpr uint32_t INLINE_GAP = 4;  // gaps up to this many cells are filled by the owning thread
+constexpr int BIN_ITEMS = 4;         // consecutive sorted slots per thread: 128-bit loads and stores on every column
+constexpr uint32_t INLINE_GAP = 4;   // gaps up to this many cells are filled by the owning thread
+
+// the whole warp fills cell_lo[lo..hi] = v for every lane that has a long gap (warp-synchronous, no shared memory)
+__device__ __forceinline__ void warp_fill(uint32_t* __restrict__ cell_lo, bool mine, uint32_t lo, uint32_t hi,
+                                          uint32_t v, int lane) {
+    uint32_t bal = __ballot_sync(0xffffffffu, mine);
+    while (bal) {
+        const int src = __ffs(bal) - 1;
+        bal &= bal - 1u;
+        const uint32_t lo_ = __shfl_sync(0xffffffffu, lo, src), hi_ = __shfl_sync(0xffffffffu, hi, src),
+                       v_ = __shfl_sync(0xffffffffu, v, src);
+        for (unsigned long long c = (unsigned long long)lo_ + lane; c <= hi_; c += 32ull) cell_lo[c] = v_;
+    }
+}
 
 __global__ void __launch_bounds__(BIN_THREADS) k_reorder(const AxgParams p) {
-    __shared__ uint32_t s_qlo[2 * BIN_THREADS], s_qhi[2 * BIN_THREADS], s_qval[2 * BIN_THREADS];
-    __shared__ uint32_t s_qn;
     const AxgDev* dev = p.dev;
     const uint32_t n = dev->n_live;
     const uint32_t* __restrict__ keys = p.skey[p.final_buf];
     const uint32_t* __restrict__ perm = p.sidx[p.final_buf];
+    const float4* __restrict__ rec = p.Brec;
     uint32_t* __restrict__ cell_lo = p.cell_lo;
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31;
 
     if (n == 0u) {  // nothing alive: every prefix is 0
         for (uint32_t c = blockIdx.x * BIN_THREADS + tid; c <= p.cells; c += gridDim.x * BIN_THREADS) cell_lo[c] = 0u;
         return;
     }
-    const uint32_t n_round = (n + BIN_THREADS - 1) / BIN_THREADS;
-    for (uint32_t r = blockIdx.x; r < n_round; r += gridDim.x) {
-        if (tid == 0) s_qn = 0u;
-        __syncthreads();
-        const uint32_t j = r * BIN_THREADS + tid;
-        if (j < n) {
-            const uint32_t k = __ldg(keys + j);
-            const uint32_t src = __ldg(perm + j);
-            // O5: A[j] = B[perm[j]]
-            p.A.x[j] = __ldg(p.B.x + src);
-            p.A.y[j] = __ldg(p.B.y + src);
-            p.A.z[j] = __ldg(p.B.z + src);
-            p.A.id[j] = __ldg(p.B.id + src);
-            p.A.species[j] = __ldg(p.B.species + src);
-            // O6 as prefix counts: cells (k_prev, k] have exactly j particles below them
-            const uint32_t lo = (j == 0u) ? 0u : __ldg(keys + j - 1) + 1u;
-            if (lo <= k) {
-                if (k - lo < INLINE_GAP) {
-                    for (uint32_t c = lo; c <= k; ++c) cell_lo[c] = j;
-                } else {
-                    const uint32_t q = atomicAdd(&s_qn, 1u);
-                    s_qlo[q] = lo; s_qhi[q] = k; s_qval[q] = j;
+    const uint32_t n_groups = (n + BIN_ITEMS - 1) / BIN_ITEMS;
+    // warp-uniform trip count: g0 is the group of lane 0
+    for (uint32_t g0 = blockIdx.x * BIN_THREADS + (tid & ~31); g0 < n_groups; g0 += gridDim.x * BIN_THREADS) {
+        const uint32_t grp = g0 + lane;
+        const uint32_t j0 = grp * BIN_ITEMS;
+        const bool full = grp < n_groups && j0 + BIN_ITEMS <= n;
+        uint32_t k[BIN_ITEMS], v[BIN_ITEMS];
+        if (full) {
+            const uint4 kk = __ldg(reinterpret_cast<const uint4*>(keys + j0));
+            const uint4 vv = __ldg(reinterpret_cast<const uint4*>(perm + j0));
+            k[0] = kk.x; k[1] = kk.y; k[2] = kk.z; k[3] = kk.w;
+            v[0] = vv.x; v[1] = vv.y; v[2] = vv.z; v[3] = vv.w;
+        } else {
+#pragma unroll
+            for (int i = 0; i < BIN_ITEMS; ++i) {
+                const bool ok = grp < n_groups && j0 + i < n;
+                k[i] = ok ? __ldg(keys + j0 + i) : 0u;
+                v[i] = ok ? __ldg(perm + j0 + i) : 0u;
+            }
+        }
+        // O5: A[j] = B[perm[j]] -- one 16 B record gather per particle, species from the top bits of the value
+        float4 r[BIN_ITEMS];
+#pragma unroll
+        for (int i = 0; i < BIN_ITEMS; ++i)
+            r[i] = (grp < n_groups && j0 + i < n) ? __ldg(rec + (v[i] & AXG_IDX_MASK)) : make_float4(0.f, 0.f, 0.f, 0.f);
+        if (full) {
+            *reinterpret_cast<float4*>(p.A.x + j0) = make_float4(r[0].x, r[1].x, r[2].x, r[3].x);
+            *reinterpret_cast<float4*>(p.A.y + j0) = make_float4(r[0].y, r[1].y, r[2].y, r[3].y);
+            *reinterpret_cast<float4*>(p.A.z + j0) = make_float4(r[0].z, r[1].z, r[2].z, r[3].z);
+            *reinterpret_cast<float4*>(p.A.id + j0) = make_float4(r[0].w, r[1].w, r[2].w, r[3].w);
+            *reinterpret_cast<uchar4*>(p.A.species + j0) =
+                make_uchar4((unsigned char)(v[0] >> 30), (unsigned char)(v[1] >> 30), (unsigned char)(v[2] >> 30),
+                            (unsigned char)(v[3] >> 30));
+        } else {
+#pragma unroll
+            for (int i = 0; i < BIN_ITEMS; ++i)
+                if (grp < n_groups && j0 + i < n) {
+                    p.A.x[j0 + i] = r[i].x;
+                    p.A.y[j0 + i] = r[i].y;
+                    p.A.z[j0 + i] = r[i].z;
+                    p.A.id[j0 + i] = __float_as_uint(r[i].w);
+                    p.A.species[j0 + i] = (uint8_t)(v[i] >> 30);
                 }
-            }
-            if (j == n - 1u) {  // cells above the last key, and the end sentinel cell_lo[cells] = n
-                const uint32_t q = atomicAdd(&s_qn, 1u);
-                s_qlo[q] = k + 1u; s_qhi[q] = p.cells; s_qval[q] = n;
-            }
         }
-        __syncthreads();
-        const uint32_t qn = s_qn;
-        for (uint32_t q = 0; q < qn; ++q) {  // long gaps: the whole block fills, coalesced
-            const uint32_t lo = s_qlo[q], hi = s_qhi[q], v = s_qval[q];
-            for (uint32_t c = lo + tid; c <= hi && c >= lo; c += BIN_THREADS) cell_lo[c] = v;
+        // O6 as prefix counts: cells (k_prev, k] have exactly j particles below them
+        uint32_t kprev = __shfl_up_sync(0xffffffffu, k[BIN_ITEMS - 1], 1);
+        if (lane == 0) kprev = (j0 > 0u && j0 - 1u < n) ? __ldg(keys + j0 - 1u) : 0u;
+#pragma unroll
+        for (int i = 0; i < BIN_ITEMS; ++i) {
+            const uint32_t j = j0 + i;
+            const bool ok = grp < n_groups && j < n;
+            const uint32_t lo = (j == 0u) ? 0u : kprev + 1u;
+            const bool gap = ok && lo <= k[i];
+            const bool lng = gap && (k[i] - lo >= INLINE_GAP);
+            if (gap && !lng)
+                for (uint32_t c = lo; c <= k[i]; ++c) cell_lo[c] = j;
+            warp_fill(cell_lo, lng, lo, k[i], j, lane);
+            // cells above the last key, and the end sentinel cell_lo[cells] = n
+            warp_fill(cell_lo, ok && j == n - 1u, k[i] + 1u, p.cells, n, lane);
+            kprev = k[i];
         }
-        __syncthreads();
     }
+}
+
+// read path: one column of the pre-sort records (0..2 = x, y, z as f32 bits, 3 = id), and the permutation without
+// the species bits
+__global__ void k_pre_export(const AxgParams p, int component, uint32_t* __restrict__ dst) {
+    const uint32_t n = p.dev->n_live;
+    const uint32_t* __restrict__ src = reinterpret_cast<const uint32_t*>(p.Brec);
+    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
+        dst[i] = src[(size_t)i * 4 + component];
+}
+__global__ void k_perm_export(const AxgParams p, uint32_t* __restrict__ dst) {
+    const uint32_t n = p.dev->n_live;
+    const uint32_t* __restrict__ src = p.sidx[p.final_buf];
+    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
+        dst[i] = src[i] & AXG_IDX_MASK;
 }
 
 // cellStart / cellEnd in the paper's convention from cell_lo (read path only)
@@ -78,6 +131,13 @@ __global__ void k_cell_export(const AxgParams p, uint32_t* __restrict__ start, u
 }  // namespace
 
 void axg_launch_reorder(const AxgParams& p, int grid, cudaStream_t s) { k_reorder<<<grid, BIN_THREADS, 0, s>>>(p); }
+
+void axg_launch_pre_export(const AxgParams& p, int component, uint32_t* dst, cudaStream_t s) {
+    k_pre_export<<<148 * 8, 256, 0, s>>>(p, component, dst);
+}
+void axg_launch_perm_export(const AxgParams& p, uint32_t* dst, cudaStream_t s) {
+    k_perm_export<<<148 * 8, 256, 0, s>>>(p, dst);
+}
 
 void axg_launch_cell_export(const AxgParams& p, uint32_t* start, uint32_t* end, cudaStream_t s) {
     k_cell_export<<<148 * 8, 256, 0, s>>>(p, start, end);

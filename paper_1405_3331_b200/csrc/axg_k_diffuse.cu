@@ -135,11 +135,8 @@ __global__ void __launch_bounds__(DIFF_THREADS, 3) k_diffuse(const AxgParams p) 
             if (a) {
                 const uint32_t o = out + __popc(b & lt);
                 const uint32_t key = cell_key(p, x[i], y[i], z[i]);
-                p.B.x[o] = x[i];
-                p.B.y[o] = y[i];
-                p.B.z[o] = z[i];
-                p.B.id[o] = id[i];
-                p.B.species[o] = (uint8_t)((sp_pack[i >> 2] >> (8 * (i & 3))) & 0xffu);
+                p.Brec[o] = make_float4(x[i], y[i], z[i], __uint_as_float(id[i]));
+                p.Bsp[o] = (uint8_t)((sp_pack[i >> 2] >> (8 * (i & 3))) & 0xffu);
                 p.key_pre[o] = key;
                 hist_add(s_hist, p.n_pass, key);
             }
@@ -169,11 +166,8 @@ __global__ void __launch_bounds__(256) k_rekey(const AxgParams p) {
     for (uint32_t g = blockIdx.x * blockDim.x + threadIdx.x; g < n; g += gridDim.x * blockDim.x) {
         const float x = p.A.x[g], y = p.A.y[g], z = p.A.z[g];
         const uint32_t key = cell_key(p, x, y, z);
-        p.B.x[g] = x;
-        p.B.y[g] = y;
-        p.B.z[g] = z;
-        p.B.id[g] = p.A.id[g];
-        p.B.species[g] = p.A.species[g];
+        p.Brec[g] = make_float4(x, y, z, __uint_as_float(p.A.id[g]));
+        p.Bsp[g] = p.A.species[g];
         p.key_pre[g] = key;
         hist_add(s_hist, p.n_pass, key);
     }
@@ -211,11 +205,8 @@ __global__ void __launch_bounds__(EMIT_THREADS) k_emit(const AxgParams p, int do
             const AxgSourceDev sd = p.src[s];
             const uint32_t o = n_surv + e;
             const uint32_t key = cell_key(p, sd.x, sd.y, sd.z);
-            p.B.x[o] = sd.x;
-            p.B.y[o] = sd.y;
-            p.B.z[o] = sd.z;
-            p.B.species[o] = (uint8_t)(sd.species_polarity & 0xffu);
-            p.B.id[o] = next_id + p.src_id_prefix[s] + j;
+            p.Brec[o] = make_float4(sd.x, sd.y, sd.z, __uint_as_float(next_id + p.src_id_prefix[s] + j));
+            p.Bsp[o] = (uint8_t)(sd.species_polarity & 0xffu);
             p.key_pre[o] = key;
             hist_add(s_hist, p.n_pass, key);
         }

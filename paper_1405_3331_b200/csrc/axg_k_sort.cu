@@ -51,13 +51,30 @@ k_sort_pass(const AxgParams p, const int pass, const uint32_t* __restrict__ kin,
         for (int i = 0; i < SORT_ITEMS; ++i) {
             const uint32_t g = first + i * 32;
             key[i] = (g < n) ? __ldg(kin + g) : 0xffffffffu;
-            val[i] = FIRST ? g : ((g < n) ? __ldg(vin + g) : 0u);
+            if (FIRST) {  // value = pre-sort index | species << 30 (the species byte rides along to P2c)
+                val[i] = (g < n) ? (g | ((uint32_t)__ldg(p.Bsp + g) << 30)) : 0u;
+            } else {
+                val[i] = (g < n) ? __ldg(vin + g) : 0u;
+            }
         }
-        // ---- rank inside the warp chunk, in memory order (item, lane) ------------------------------------
+        // ---- lanes with the same digit, by 8 ballots per item (independent across items: no MATCH latency chain)
 #pragma unroll
         for (int i = 0; i < SORT_ITEMS; ++i) {
             const uint32_t d = (key[i] >> shift) & 0xffu;
-            const uint32_t m = __match_any_sync(0xffffffffu, d);
+            uint32_t m = 0xffffffffu;
+#pragma unroll
+            for (int b = 0; b < 8; ++b) {
+                const bool bit = (d >> b) & 1u;
+                const uint32_t bal = __ballot_sync(0xffffffffu, bit);
+                m &= bit ? bal : ~bal;
+            }
+            rank[i] = m;
+        }
+        // ---- rank inside the warp chunk, in memory order (item, lane): per-warp digit counters in shared memory
+#pragma unroll
+        for (int i = 0; i < SORT_ITEMS; ++i) {
+            const uint32_t d = (key[i] >> shift) & 0xffu;
+            const uint32_t m = rank[i];
             const int leader = __ffs(m) - 1;
             uint32_t old = 0u;
             if (lane == leader) {
@@ -69,7 +86,9 @@ k_sort_pass(const AxgParams p, const int pass, const uint32_t* __restrict__ kin,
             rank[i] = old + __popc(m & lt);
         }
         __syncthreads();
-        // ---- per digit: scan over warps, scan over digits, look-back over tiles ----------------------------
+        // ---- per digit: scan over warps, scan over digits, publish the tile aggregate ---------------------------
+        uint32_t count = 0u;
+        unsigned long long* st = p.sort_state + (size_t)tile * AXG_RADIX + tid;
         if (tid < AXG_RADIX) {
             const int d = tid;
             uint32_t run = 0u;
@@ -79,8 +98,7 @@ k_sort_pass(const AxgParams p, const int pass, const uint32_t* __restrict__ kin,
                 s_wh[w * AXG_RADIX + d] = run;
                 run += c;
             }
-            const uint32_t count = run;
-            unsigned long long* st = p.sort_state + (size_t)tile * AXG_RADIX + d;
+            count = run;
             axg_st_state(st, axg_pack(epoch, tile == 0 ? AXG_FLAG_INCL : AXG_FLAG_AGG, count));
             uint32_t inc = count;
 #pragma unroll
@@ -92,8 +110,20 @@ k_sort_pass(const AxgParams p, const int pass, const uint32_t* __restrict__ kin,
             asm volatile("bar.sync 1, 256;");  // the 8 warps that own the digits
             uint32_t off = 0u;
             for (int w = 0; w < warp; ++w) off += s_misc[1 + w];
-            const uint32_t dstart = off + inc - count;
-            s_dstart[d] = dstart;
+            s_dstart[d] = off + inc - count;
+        }
+        __syncthreads();
+        // ---- sort the tile through shared memory (gives the predecessors time before the look-back) -------------
+#pragma unroll
+        for (int i = 0; i < SORT_ITEMS; ++i) {
+            const uint32_t d = (key[i] >> shift) & 0xffu;
+            const uint32_t pos = s_dstart[d] + my_wh[d] + rank[i];
+            s_key[pos] = key[i];
+            s_val[pos] = val[i];
+        }
+        // ---- decoupled look-back over the predecessor tiles, one thread per digit ------------------------------
+        if (tid < AXG_RADIX) {
+            const int d = tid;
             uint32_t excl = 0u;
             if (tile > 0) {
                 for (int q = (int)tile - 1;; --q) {
@@ -108,16 +138,7 @@ k_sort_pass(const AxgParams p, const int pass, const uint32_t* __restrict__ kin,
                 }
                 axg_st_state(st, axg_pack(epoch, AXG_FLAG_INCL, excl + count));
             }
-            s_gbase[d] = dev->base[pass][d] + excl - dstart;
-        }
-        __syncthreads();
-        // ---- sort the tile through shared memory ----------------------------------------------------------
-#pragma unroll
-        for (int i = 0; i < SORT_ITEMS; ++i) {
-            const uint32_t d = (key[i] >> shift) & 0xffu;
-            const uint32_t pos = s_dstart[d] + my_wh[d] + rank[i];
-            s_key[pos] = key[i];
-            s_val[pos] = val[i];
+            s_gbase[d] = dev->base[pass][d] + excl - s_dstart[d];
         }
         __syncthreads();
         const uint32_t tile_n = min((uint32_t)SORT_TILE, n - tile * SORT_TILE);
