@@ -108,8 +108,11 @@ def use_torch_allocator():
             return None
 
     def _free(ptr, _user):
-        if ptr:
-            torch.cuda.caching_allocator_delete(int(ptr))
+        try:
+            if ptr:
+                torch.cuda.caching_allocator_delete(int(ptr))
+        except Exception:      # interpreter shutdown: torch is already gone, the process is about to free everything
+            pass
 
     _hooks = (_ALLOC_T(_alloc), _FREE_T(_free))
     rc = lib().axg_set_allocator(_hooks[0], _hooks[1], None)

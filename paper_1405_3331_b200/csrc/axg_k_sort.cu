@@ -2,7 +2,7 @@
 // (DESIGN.md §3 O4, reading A-9).  The paper sorts (cell hash, particle id) pairs with a
 // library radix sort; this is a hand-written single-pass-per-digit ("onesweep"-style) sort:
 //   - digit histograms of ALL passes are known before the first pass (accumulated by k_diffuse / k_emit),
-//   - inside a tile every warp ranks its keys in memory order with __match_any_sync + popc (stable),
+//   - inside a tile every warp ranks its keys in memory order by warp ballots + popc (stable),
 //   - per-tile per-digit counts chain across tiles by decoupled look-back (one 64-bit word per tile and digit,
 //     epoch-tagged so the words never need clearing),
 //   - the tile is sorted through shared memory so that global stores run along digit runs.
@@ -35,28 +35,34 @@ k_sort_pass(const AxgParams p, const int pass, const uint32_t* __restrict__ kin,
     const uint32_t lt = axg_lanemask_lt();
     const int shift = 8 * pass;
     uint32_t* my_wh = s_wh + warp * AXG_RADIX;
+    uint32_t* s_tk = s_misc + 12;  // [2] tile tickets, double-buffered: the next ticket is drawn a tile ahead
 
-    while (true) {
-        __syncthreads();
-        if (tid == 0) s_misc[0] = atomicAdd(&dev->ticket, 1u);
-#pragma unroll
-        for (int i = 0; i < AXG_RADIX / 32; ++i) my_wh[i * 32 + lane] = 0u;
-        __syncthreads();
-        const uint32_t tile = s_misc[0];
-        if (tile >= n_tiles) break;
-
+    uint32_t key[SORT_ITEMS], val[SORT_ITEMS], rank[SORT_ITEMS];
+    auto load_tile = [&](uint32_t tile) {
         const uint32_t first = tile * SORT_TILE + warp * (32 * SORT_ITEMS) + lane;
-        uint32_t key[SORT_ITEMS], val[SORT_ITEMS], rank[SORT_ITEMS];
 #pragma unroll
         for (int i = 0; i < SORT_ITEMS; ++i) {
             const uint32_t g = first + i * 32;
-            key[i] = (g < n) ? __ldg(kin + g) : 0xffffffffu;
+            const bool ok = tile < n_tiles && g < n;
+            key[i] = ok ? __ldg(kin + g) : 0xffffffffu;
             if (FIRST) {  // value = pre-sort index | species << 30 (the species byte rides along to P2c)
-                val[i] = (g < n) ? (g | ((uint32_t)__ldg(p.Bsp + g) << 30)) : 0u;
+                val[i] = ok ? (g | ((uint32_t)__ldg(p.Bsp + g) << 30)) : 0u;
             } else {
-                val[i] = (g < n) ? __ldg(vin + g) : 0u;
+                val[i] = ok ? __ldg(vin + g) : 0u;
             }
         }
+    };
+
+#pragma unroll
+    for (int i = 0; i < AXG_RADIX / 32; ++i) my_wh[i * 32 + lane] = 0u;
+    if (tid == 0) s_tk[0] = atomicAdd(&dev->ticket, 1u);
+    __syncthreads();
+    uint32_t tile = s_tk[0];
+    int par = 0;
+    load_tile(tile);
+
+    while (tile < n_tiles) {
+        if (tid == 0) s_tk[par ^ 1] = atomicAdd(&dev->ticket, 1u);  // read by everyone after barrier B
         // ---- lanes with the same digit, by 8 ballots per item (independent across items: no MATCH latency chain)
 #pragma unroll
         for (int i = 0; i < SORT_ITEMS; ++i) {
@@ -85,7 +91,7 @@ k_sort_pass(const AxgParams p, const int pass, const uint32_t* __restrict__ kin,
             old = __shfl_sync(0xffffffffu, old, leader);
             rank[i] = old + __popc(m & lt);
         }
-        __syncthreads();
+        __syncthreads();  // barrier A
         // ---- per digit: scan over warps, scan over digits, publish the tile aggregate ---------------------------
         uint32_t count = 0u;
         unsigned long long* st = p.sort_state + (size_t)tile * AXG_RADIX + tid;
@@ -112,8 +118,8 @@ k_sort_pass(const AxgParams p, const int pass, const uint32_t* __restrict__ kin,
             for (int w = 0; w < warp; ++w) off += s_misc[1 + w];
             s_dstart[d] = off + inc - count;
         }
-        __syncthreads();
-        // ---- sort the tile through shared memory (gives the predecessors time before the look-back) -------------
+        __syncthreads();  // barrier B
+        // ---- sort the tile through shared memory; the warp's counter row is zeroed for the next tile ------------
 #pragma unroll
         for (int i = 0; i < SORT_ITEMS; ++i) {
             const uint32_t d = (key[i] >> shift) & 0xffu;
@@ -121,26 +127,46 @@ k_sort_pass(const AxgParams p, const int pass, const uint32_t* __restrict__ kin,
             s_key[pos] = key[i];
             s_val[pos] = val[i];
         }
-        // ---- decoupled look-back over the predecessor tiles, one thread per digit ------------------------------
+        __syncwarp();
+#pragma unroll
+        for (int i = 0; i < AXG_RADIX / 32; ++i) my_wh[i * 32 + lane] = 0u;
+        // ---- the registers are free: prefetch the next tile while the look-back and the write-out run ----------
+        const uint32_t next_tile = s_tk[par ^ 1];
+        load_tile(next_tile);
+        // ---- decoupled look-back over the predecessor tiles, one thread per digit, 4 predecessors per probe -----
         if (tid < AXG_RADIX) {
             const int d = tid;
             uint32_t excl = 0u;
             if (tile > 0) {
-                for (int q = (int)tile - 1;; --q) {
-                    unsigned long long w;
-                    uint32_t f;
-                    do {
-                        w = axg_ld_state(p.sort_state + (size_t)q * AXG_RADIX + d);
-                        f = axg_flag(w, epoch);
-                    } while (f == 0u);
-                    excl += (uint32_t)w;
-                    if (f == (uint32_t)AXG_FLAG_INCL) break;
+                int q = (int)tile - 1;
+                const unsigned long long* base = p.sort_state + d;
+                const unsigned long long zero_incl = axg_pack(epoch, AXG_FLAG_INCL, 0u);
+                while (true) {
+                    unsigned long long w[4];
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+                        w[j] = (q - j >= 0) ? axg_ld_state(base + (size_t)(q - j) * AXG_RADIX) : zero_incl;
+                    bool done = false;
+                    int adv = 0;
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        if (!done && adv == j) {
+                            const uint32_t f = axg_flag(w[j], epoch);
+                            if (f != 0u) {
+                                excl += (uint32_t)w[j];
+                                adv = j + 1;
+                                done = (f == (uint32_t)AXG_FLAG_INCL);
+                            }
+                        }
+                    }
+                    if (done) break;
+                    q -= adv;
                 }
                 axg_st_state(st, axg_pack(epoch, AXG_FLAG_INCL, excl + count));
             }
             s_gbase[d] = dev->base[pass][d] + excl - s_dstart[d];
         }
-        __syncthreads();
+        __syncthreads();  // barrier C
         const uint32_t tile_n = min((uint32_t)SORT_TILE, n - tile * SORT_TILE);
 #pragma unroll
         for (int i = 0; i < SORT_ITEMS; ++i) {
@@ -152,6 +178,10 @@ k_sort_pass(const AxgParams p, const int pass, const uint32_t* __restrict__ kin,
                 vout[g] = s_val[pos];
             }
         }
+        tile = next_tile;
+        par ^= 1;
+        // no barrier here: the next tile's shared-memory writes (s_wh scan, s_key scatter, s_gbase) all sit behind
+        // its barriers A / B, which every thread reaches only after it has finished this write-out
     }
     if (axg_last_block(dev) && tid == 0) {
         dev->ticket = 0u;
