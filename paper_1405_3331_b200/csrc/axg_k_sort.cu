@@ -16,6 +16,23 @@ constexpr int SORT_WARPS = SORT_THREADS / 32;
 constexpr int SORT_TILE = SORT_THREADS * SORT_ITEMS;
 constexpr size_t SORT_SMEM = (size_t)(2 * SORT_TILE + SORT_WARPS * AXG_RADIX + 2 * AXG_RADIX + 16) * sizeof(uint32_t);
 
+// One bit of the peer search: keep in m the lanes whose digit agrees with mine on `bitmask`.  Four instructions
+// (LOP3 -> predicate, VOTE, two predicated LOP3: m & b / m & ~b); the C++ form `m &= bit ? bal : ~bal` compiled to seven.
+__device__ __forceinline__ uint32_t peers_step(uint32_t m, uint32_t d, uint32_t bitmask) {
+    asm("{\n\t"
+        ".reg .pred p;\n\t"
+        ".reg .b32 t, b;\n\t"
+        "and.b32 t, %1, %2;\n\t"
+        "setp.ne.u32 p, t, 0;\n\t"
+        "vote.sync.ballot.b32 b, p, 0xffffffff;\n\t"
+        "@p and.b32 %0, %0, b;\n\t"
+        "@!p lop3.b32 %0, %0, b, 0, 0x30;\n\t"
+        "}"
+        : "+r"(m)
+        : "r"(d), "r"(bitmask));
+    return m;
+}
+
 template <bool FIRST>
 __global__ void __launch_bounds__(SORT_THREADS, 2)
 k_sort_pass(const AxgParams p, const int pass, const uint32_t* __restrict__ kin, const uint32_t* __restrict__ vin,
@@ -69,11 +86,7 @@ k_sort_pass(const AxgParams p, const int pass, const uint32_t* __restrict__ kin,
             const uint32_t d = (key[i] >> shift) & 0xffu;
             uint32_t m = 0xffffffffu;
 #pragma unroll
-            for (int b = 0; b < 8; ++b) {
-                const bool bit = (d >> b) & 1u;
-                const uint32_t bal = __ballot_sync(0xffffffffu, bit);
-                m &= bit ? bal : ~bal;
-            }
+            for (int b = 0; b < 8; ++b) m = peers_step(m, d, 1u << b);
             rank[i] = m;
         }
         // ---- rank inside the warp chunk, in memory order (item, lane): per-warp digit counters in shared memory
