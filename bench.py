@@ -66,18 +66,30 @@ def key_passes(cells):
     return (bits + 7) // 8
 
 
-def bytes_model(w, n_live, n_active_cones, n_stencil):
-    """Algorithmic bytes of ONE step at n_live particles, per kernel."""
+def bytes_model(w, n_live, n_active_cones, n_stencil, count_mode):
+    """Algorithmic bytes of ONE step at n_live particles.  `step` is SURVEY.md §8(d)'s figure for the
+    METHOD (K1 38 + sort 12 + 16 (passes - 1) + reorder 42 per particle, 8 B per cell of cell-range upkeep, the cone
+    bytes) and does not depend on how P2 is computed; the per-kernel entries are what each kernel of the chosen
+    binning mode must move itself."""
     passes = key_passes(w.cells)
     two_species = len({s[3] for s in w.sources}) > 1
     per_cone = n_stencil * 8 + 90 + 12 + (n_stencil * 1 if two_species else 0)
-    return {
-        "diffuse": 38.0 * n_live,                       # 17 B read + 17 B write + 4 B key
-        "sort": (12.0 + 16.0 * (passes - 1)) * n_live,  # pass 0: 4 read + 8 write; later passes 8 + 8
-        "sort_launches": passes,
-        "reorder": 42.0 * n_live + 4.0 * w.cells,       # perm 4 + key 4 + gather 17 + write 17; cell ranges 4 B / cell
-        "sense": float(per_cone) * n_active_cones,
-    }
+    sense = float(per_cone) * n_active_cones
+    step = (38.0 + 12.0 + 16.0 * (passes - 1) + 42.0) * n_live + 8.0 * w.cells + sense
+    if count_mode:
+        k = {"diffuse": (38.0 + 8.0) * n_live,   # + 4 B atomic on cnt[key] + 4 B arrival number
+             "scan": 8.0 * (w.cells + 1),         # read cnt, write cell_lo
+             "place": 17.0 * n_live,              # key 4 + arrival 4 + species 1 + cell_lo 4, slot write 4
+             "settle": 61.0 * n_live,             # slot 4 + record 16 + cell_lo 8 + SoA 17 + key 4 + perm 4 + cnt 4 + cell 4
+             "sense": sense}
+        launches = {"diffuse": 1, "scan": 1, "place": 1, "settle": 1, "sense": 1}
+    else:
+        k = {"diffuse": 38.0 * n_live,
+             "sort": (12.0 + 16.0 * (passes - 1)) * n_live,   # pass 0: 4 read + 8 write; later passes 8 + 8
+             "reorder": 42.0 * n_live + 4.0 * w.cells,        # perm 4 + key 4 + gather 17 + write 17; 4 B / cell
+             "sense": sense}
+        launches = {"diffuse": 1, "sort": passes, "reorder": 1, "sense": 1}
+    return step, k, launches
 
 
 class ClockSampler:
@@ -221,8 +233,12 @@ def run_ours(args, w):
     w.max_segments = Wm + 2 * K + e2e_steps + 8
     seed = w.seed
 
+    bin_req = {"auto": axg.BIN_AUTO, "radix": axg.BIN_RADIX, "count": axg.BIN_COUNT}[args.binning]
+    count_mode = bin_req == axg.BIN_COUNT or (bin_req == axg.BIN_AUTO and w.cells <= 4 * (w.max_particles or 1 << 20))
+
     def make_sim(D, emission):
         sim_ = axg.Axg(w.grid, D, emission, w.radius, w.speed, w.noise, seed)
+        sim_.set_binning(bin_req)
         if world > 1:
             sim_.set_shard(rank, world)   # every rank pre-runs its own shard: particle sets of sources never interact
         return sim_
@@ -295,11 +311,11 @@ def run_ours(args, w):
                     if dx * dx + dy * dy + dz * dz <= r2)
     extra = {}
     if ktimes is not None:
-        bm = bytes_model(w, n_avg, active, n_stencil)
+        step_bytes, bm, launches_of = bytes_model(w, n_avg, active, n_stencil, count_mode)
         per_step_ms = {k: v / K for k, v in ktimes.items()}
-        launches_of = {"diffuse": 1, "sort": bm["sort_launches"], "reorder": 1, "sense": 1}
-        kernel_name = {"diffuse": "k_diffuse", "sort": "k_sort_pass", "reorder": "k_reorder", "sense": "k_sense"}
-        dom = max(("diffuse", "sort", "reorder", "sense"), key=lambda k: per_step_ms[k])
+        kernel_name = {"diffuse": "k_diffuse", "sort": "k_sort_pass", "reorder": "k_reorder", "sense": "k_sense",
+                       "scan": "k_cell_scan", "place": "k_place", "settle": "k_settle"}
+        dom = max(bm.keys(), key=lambda k: per_step_ms[k])
         per_launch_ms = per_step_ms[dom] / launches_of[dom]
         per_launch_bytes = bm[dom] / launches_of[dom]
         achieved = per_launch_bytes / (per_launch_ms * 1e-3) / 1e9
@@ -308,18 +324,15 @@ def run_ours(args, w):
                 "peak_source": peak_src, "launches_per_step": launches_of[dom],
                 "algorithmic_bytes_per_launch": per_launch_bytes, "ms_per_launch": per_launch_ms,
                 "share_of_step": per_step_ms[dom] / max(sum(per_step_ms.values()), 1e-12)}
-        step_bytes = bm["diffuse"] + bm["sort"] + bm["reorder"] + bm["sense"]
         step_ms = ms / K
         step_gbs = step_bytes / (step_ms * 1e-3) / 1e9
         extra["roofline_step"] = {"achieved": step_gbs, "unit": "GB/s", "frac_of_measured_copy": step_gbs / peak,
                                   "frac_of_nominal_8TBs": step_gbs / NOMINAL_GBS,
                                   "algorithmic_bytes_per_particle": step_bytes / max(n_avg, 1)}
-        extra["kernels_ms_per_step"] = {k: round(v, 5) for k, v in per_step_ms.items()}
-        extra["kernels_gbs"] = {k: bm[k] / (per_step_ms[k] * 1e-3) / 1e9 for k in ("diffuse", "sort", "reorder")
-                                if per_step_ms[k] > 0}
-        sort_ms = per_step_ms["sort"]
-        extra["sort_keys_per_s"] = n_avg / (sort_ms * 1e-3) if sort_ms > 0 else None
+        extra["kernels_ms_per_step"] = {k: round(v, 5) for k, v in per_step_ms.items() if v > 0}
+        extra["kernels_gbs"] = {k: bm[k] / (per_step_ms[k] * 1e-3) / 1e9 for k in bm if per_step_ms[k] > 0}
         extra["cone_steps_per_s"] = active / (step_ms * 1e-3)
+        extra["binning"] = "count" if count_mode else "radix"
 
     # ---- e2e: the same job through the C-ABI with HOST buffers; every host<->device copy inside the timed region --
     # upload of the particle SoA + cone state from pinned host memory, then e2e_steps x [axg_step(1), read back cone
@@ -414,6 +427,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--coarse", type=int, default=16, help="coarse-time factor of the steady-state pre-run")
     ap.add_argument("--e2e-steps", type=int, default=20)
+    ap.add_argument("--binning", default="auto", choices=("auto", "radix", "count"))
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     from paper_1405_3331_b200 import workloads as W

@@ -164,6 +164,17 @@ int axg_step_phase(axg_ctx* ctx, uint32_t phase_mask);
  * AXG_CONE_MOMENT then read 0 instead of the last active value.                                           */
 int axg_set_shard(axg_ctx* ctx, uint32_t rank, uint32_t world);
 
+/* How P2 (binning) is computed; the results are identical bit for bit.
+ *  AXG_BIN_RADIX  stable LSD radix sort of (key, index), 8-bit digits, one onesweep pass per digit, then the
+ *                 reorder + cell-range kernel.  Cost ~ passes x N; independent of the number of cells.
+ *  AXG_BIN_COUNT  counting sort over the cells: P1 counts particles per cell (one L2 atomic each), a single-pass
+ *                 scan over the cells gives the cell ranges, and a rank-inside-the-cell kernel restores the stable
+ *                 order.  Cost ~ N + cells; 4 B x cells of extra device memory.
+ *  AXG_BIN_AUTO   (default) COUNT when cells <= 4 x particle capacity, else RADIX.
+ * Allowed whenever no step is half done (not between AXG_PHASE_DIFFUSE and AXG_PHASE_BIN): AXG_ESTATE.    */
+enum { AXG_BIN_AUTO = 0, AXG_BIN_RADIX = 1, AXG_BIN_COUNT = 2 };
+int axg_set_binning(axg_ctx* ctx, int mode);
+
 /* Device pointer (int32[C][AXG_MAX_SPECIES][4] = n,Mx,My,Mz) of the per-cone sensing sums, for the NCCL
  * all-reduce between P3 and P4 when sharded.  *bytes = its size.  Owned by ctx.                           */
 int axg_sense_buffer(axg_ctx* ctx, void** device_ptr, size_t* bytes);
@@ -199,7 +210,7 @@ int axg_last_step_stats(axg_ctx* ctx, float* device_ms, uint64_t* launches, uint
  * hold AXG_KERNEL_COUNT floats after the call via axg_kernel_times.                                      */
 enum {
     AXG_K_CLEAR = 0, AXG_K_DIFFUSE = 1, AXG_K_EMIT = 2, AXG_K_SORT = 3, AXG_K_REORDER = 4, AXG_K_SENSE = 5,
-    AXG_K_ADVANCE = 6, AXG_K_COMMIT = 7, AXG_KERNEL_COUNT = 8
+    AXG_K_ADVANCE = 6, AXG_K_COMMIT = 7, AXG_K_SCAN = 8, AXG_K_PLACE = 9, AXG_K_SETTLE = 10, AXG_KERNEL_COUNT = 11
 };
 int axg_profile_next_step(axg_ctx* ctx, int enable);
 int axg_kernel_times(axg_ctx* ctx, float* times_ms /* AXG_KERNEL_COUNT */);

@@ -26,12 +26,13 @@ _DTYPES = {
 }
 PHASE_DIFFUSE, PHASE_BIN, PHASE_SENSE, PHASE_ADVANCE, PHASE_COMMIT, PHASE_ALL = 1, 2, 4, 8, 16, 31
 COUNTER_NAMES = ("step", "n_live", "next_id", "emitted", "absorbed", "active", "arrived", "exited")
-KERNEL_NAMES = ("clear", "diffuse", "emit", "sort", "reorder", "sense", "advance", "commit")
+KERNEL_NAMES = ("clear", "diffuse", "emit", "sort", "reorder", "sense", "advance", "commit", "scan", "place", "settle")
+BIN_AUTO, BIN_RADIX, BIN_COUNT = 0, 1, 2
 EXPORTS = (
     "axg_create", "axg_place_neurons", "axg_add_source", "axg_step", "axg_read_state", "axg_destroy",
     "axg_last_error", "axg_set_capacity", "axg_load_particles", "axg_load_cones", "axg_step_phase", "axg_set_shard",
     "axg_sense_buffer", "axg_set_stream", "axg_set_allocator", "axg_last_step_stats", "axg_profile_next_step",
-    "axg_kernel_times", "axg_check_capacity", "axg_enqueue_phase", "axg_sync",
+    "axg_kernel_times", "axg_check_capacity", "axg_enqueue_phase", "axg_sync", "axg_set_binning",
 )
 
 _ALLOC_T = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p)
@@ -81,6 +82,7 @@ def lib(build=True):
     L.axg_check_capacity.argtypes = [vp, u32]
     L.axg_enqueue_phase.argtypes = [vp, u32]
     L.axg_sync.argtypes = [vp]
+    L.axg_set_binning.argtypes = [vp, C.c_int]
     L.axg_load_particles.argtypes = [vp, vp, vp, vp, vp, vp, u64, u32, u32]
     L.axg_load_cones.argtypes = [vp, vp, vp, vp, vp, u32]
     L.axg_read_state.argtypes = [vp, u32, vp, sz, C.POINTER(sz)]
@@ -176,6 +178,9 @@ class Axg:
 
     def add_source(self, x, y, z, species=0, polarity=1, rate=0):
         self._chk(self._L.axg_add_source(self._h, x, y, z, species, polarity, rate))
+
+    def set_binning(self, mode):
+        self._chk(self._L.axg_set_binning(self._h, int(mode)))
 
     def set_shard(self, rank, world):
         self._chk(self._L.axg_set_shard(self._h, rank, world))

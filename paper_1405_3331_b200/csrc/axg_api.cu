@@ -51,6 +51,10 @@ struct axg_ctx {
     std::vector<void*> particle_bufs;  // everything sized by max_particles
     void* d_dev = nullptr;
     void* d_cell_lo = nullptr;
+    void* d_cnt = nullptr;
+    void* d_scan_state = nullptr;
+    int bin_request = AXG_BIN_AUTO;
+    bool cnt_dirty = false;   // P1 has counted into cnt and P2 has not consumed (and re-zeroed) it yet
     void* d_src = nullptr;
     void* d_src_id_prefix = nullptr;
     void* d_src_emit_prefix = nullptr;
@@ -70,6 +74,9 @@ struct axg_ctx {
     std::vector<cudaEvent_t> prof_events;
 
     size_t cells() const { return (size_t)grid.nx * grid.ny * grid.nz; }
+    // cell arrays are padded to whole scan tiles so that 128-bit accesses of the last tile stay inside
+    size_t cells_padded() const { return ((cells() + 1 + AXG_SCAN_TILE - 1) / AXG_SCAN_TILE + 1) * AXG_SCAN_TILE; }
+    size_t scan_tiles() const { return cells_padded() / AXG_SCAN_TILE + 2; }
 };
 
 namespace {
@@ -128,7 +135,7 @@ int key_passes(size_t cells) {
 int alloc_fixed(axg_ctx* c) {
     if (c->d_dev) return AXG_OK;
     c->d_dev = dev_alloc(c, sizeof(AxgDev));
-    c->d_cell_lo = dev_alloc(c, (c->cells() + 1) * sizeof(uint32_t));
+    c->d_cell_lo = dev_alloc(c, c->cells_padded() * sizeof(uint32_t));
     c->d_src = dev_alloc(c, AXG_MAX_SOURCES * sizeof(AxgSourceDev));
     c->d_src_id_prefix = dev_alloc(c, (AXG_MAX_SOURCES + 1) * sizeof(uint32_t));
     c->d_src_emit_prefix = dev_alloc(c, (AXG_MAX_SOURCES + 1) * sizeof(uint32_t));
@@ -148,7 +155,7 @@ int alloc_fixed(axg_ctx* c) {
     if (!c->d_dev || !c->d_cell_lo || !c->d_src || !c->d_src_id_prefix || !c->d_src_emit_prefix || !c->d_stencil)
         return fail(c, AXG_ECUDA, "device allocation failed");
     CU(c, cudaMemsetAsync(c->d_dev, 0, sizeof(AxgDev), c->stream));
-    CU(c, cudaMemsetAsync(c->d_cell_lo, 0, (c->cells() + 1) * sizeof(uint32_t), c->stream));
+    CU(c, cudaMemsetAsync(c->d_cell_lo, 0, c->cells_padded() * sizeof(uint32_t), c->stream));
     CU(c, cudaMemcpyAsync(c->d_stencil, st.data(), st.size() * sizeof(int32_t), cudaMemcpyHostToDevice, c->stream));
     CU(c, cudaStreamSynchronize(c->stream));
     AxgParams& P = c->P;
@@ -185,8 +192,9 @@ int alloc_particles(axg_ctx* c, uint64_t cap, AxgParams& P, std::vector<void*>& 
     const size_t sizes[] = {n * 4, n * 4, n * 4, n, n * 4,  // A (SoA)
                             n * 16, n,                      // Brec, Bsp
                             n * 4, n * 4, n * 4, n * 4, n * 4,  // key_pre, skey[2], sidx[2]
-                            diff_tiles * 8, sort_tiles * AXG_RADIX * 8};
-    constexpr int NB = 14;
+                            diff_tiles * 8, sort_tiles * AXG_RADIX * 8,
+                            n * 4};                         // arrival
+    constexpr int NB = 15;
     void* ptr[NB];
     for (int i = 0; i < NB; ++i) {
         ptr[i] = dev_alloc(c, sizes[i]);
@@ -205,6 +213,7 @@ int alloc_particles(axg_ctx* c, uint64_t cap, AxgParams& P, std::vector<void*>& 
     P.sidx[0] = (uint32_t*)ptr[10]; P.sidx[1] = (uint32_t*)ptr[11];
     P.tile_state = (unsigned long long*)ptr[12];
     P.sort_state = (unsigned long long*)ptr[13];
+    P.arrival = (uint32_t*)ptr[14];
     P.capacity = (uint32_t)cap;
     // look-back words must not alias a live epoch: zero them (epoch 0 words with flag 0 = not ready)
     CU(c, cudaMemsetAsync(ptr[12], 0, sizes[12], c->stream));
@@ -212,14 +221,32 @@ int alloc_particles(axg_ctx* c, uint64_t cap, AxgParams& P, std::vector<void*>& 
     return AXG_OK;
 }
 
+// AXG_BIN_AUTO -> a concrete mode; the count array exists (all-zero) whenever the mode is COUNT
+int resolve_binning(axg_ctx* c) {
+    int mode = c->bin_request;
+    if (mode == AXG_BIN_AUTO) mode = (c->cells() <= 4 * (size_t)c->max_particles) ? AXG_BIN_COUNT : AXG_BIN_RADIX;
+    if (mode == AXG_BIN_COUNT && !c->d_cnt) {
+        c->d_cnt = dev_alloc(c, c->cells_padded() * sizeof(uint32_t));
+        c->d_scan_state = dev_alloc(c, c->scan_tiles() * sizeof(unsigned long long));
+        if (!c->d_cnt || !c->d_scan_state) return fail(c, AXG_ECUDA, "device allocation failed (cell counts)");
+        CU(c, cudaMemsetAsync(c->d_cnt, 0, c->cells_padded() * sizeof(uint32_t), c->stream));
+        CU(c, cudaMemsetAsync(c->d_scan_state, 0, c->scan_tiles() * sizeof(unsigned long long), c->stream));
+        c->P.cnt = (uint32_t*)c->d_cnt;
+        c->P.scan_state = (unsigned long long*)c->d_scan_state;
+    }
+    c->P.bin_mode = mode == AXG_BIN_COUNT ? AXG_BIN_COUNT_D : AXG_BIN_RADIX_D;
+    return AXG_OK;
+}
+
 int ensure_particles(axg_ctx* c) {
     int rc = alloc_fixed(c);
     if (rc) return rc;
-    if (c->particles_allocated) return AXG_OK;
-    rc = alloc_particles(c, c->max_particles, c->P, c->particle_bufs);
-    if (rc) return rc;
-    c->particles_allocated = true;
-    return AXG_OK;
+    if (!c->particles_allocated) {
+        rc = alloc_particles(c, c->max_particles, c->P, c->particle_bufs);
+        if (rc) return rc;
+        c->particles_allocated = true;
+    }
+    return resolve_binning(c);
 }
 
 void free_cones(axg_ctx* c) {
@@ -324,25 +351,43 @@ int enqueue_phases(axg_ctx* c, uint32_t mask, Prof& prof) {
     const AxgParams& P = c->P;
     cudaStream_t s = c->stream;
     int launches = 0;
+    const bool count_mode = P.bin_mode == AXG_BIN_COUNT_D;
+    auto zero_cnt_if_dirty = [&]() {  // harness orders only (P1 twice, or P2 on given positions after a P1)
+        if (count_mode && c->cnt_dirty) cudaMemsetAsync(c->d_cnt, 0, c->cells_padded() * sizeof(uint32_t), s);
+    };
     if (mask & AXG_PHASE_DIFFUSE) {
+        zero_cnt_if_dirty();
         prof.mark(AXG_K_DIFFUSE);
         axg_launch_diffuse(P, N_SM * 3, s);
         prof.mark(AXG_K_EMIT);
         axg_launch_emit(P, 1, s);
         launches += 2;
+        c->cnt_dirty = count_mode;
     }
     if (mask & AXG_PHASE_BIN) {
         if (!(mask & AXG_PHASE_DIFFUSE)) {
+            zero_cnt_if_dirty();
             prof.mark(AXG_K_EMIT);
             axg_launch_rekey(P, N_SM * 8, s);
             axg_launch_emit(P, 0, s);
             launches += 2;
         }
-        prof.mark(AXG_K_SORT);
-        for (int q = 0; q < P.n_pass; ++q) axg_launch_sort_pass(P, q, N_SM * 2, s);
-        prof.mark(AXG_K_REORDER);
-        axg_launch_reorder(P, N_SM * 8, s);
-        launches += P.n_pass + 1;
+        if (count_mode) {
+            prof.mark(AXG_K_SCAN);
+            axg_launch_cell_scan(P, N_SM * 4, s);
+            prof.mark(AXG_K_PLACE);
+            axg_launch_place(P, N_SM * 8, s);
+            prof.mark(AXG_K_SETTLE);
+            axg_launch_settle(P, N_SM * 6, s);
+            launches += 3;
+            c->cnt_dirty = false;
+        } else {
+            prof.mark(AXG_K_SORT);
+            for (int q = 0; q < P.n_pass; ++q) axg_launch_sort_pass(P, q, N_SM * 2, s);
+            prof.mark(AXG_K_REORDER);
+            axg_launch_reorder(P, N_SM * 8, s);
+            launches += P.n_pass + 1;
+        }
     }
     if ((mask & AXG_PHASE_SENSE) && P.n_cones) {
         prof.mark(AXG_K_SENSE);
@@ -433,6 +478,7 @@ AXG_API void axg_destroy(axg_ctx* c) {
     cudaStreamSynchronize(c->stream);
     free_particles(c);
     free_cones(c);
+    dev_free(c->d_cnt); dev_free(c->d_scan_state);
     dev_free(c->d_dev); dev_free(c->d_cell_lo); dev_free(c->d_src); dev_free(c->d_src_id_prefix);
     dev_free(c->d_src_emit_prefix); dev_free(c->d_stencil);
     for (cudaEvent_t e : c->prof_events) cudaEventDestroy(e);
@@ -455,6 +501,13 @@ AXG_API int axg_set_shard(axg_ctx* c, uint32_t rank, uint32_t world) {
     c->shard_rank = rank; c->shard_world = world;
     c->P.sharded = world > 1 ? 1 : 0;
     return upload_sources(c);
+}
+
+AXG_API int axg_set_binning(axg_ctx* c, int mode) {
+    if (!c || (mode != AXG_BIN_AUTO && mode != AXG_BIN_RADIX && mode != AXG_BIN_COUNT)) return fail(c, AXG_EINVAL, "bad binning mode");
+    if (c->cnt_dirty) return fail(c, AXG_ESTATE, "a step is half done (P1 without P2)");
+    c->bin_request = mode;
+    return c->particles_allocated ? resolve_binning(c) : AXG_OK;
 }
 
 AXG_API int axg_add_source(axg_ctx* c, float x, float y, float z, uint8_t species, int8_t polarity, uint32_t rate) {
@@ -545,7 +598,7 @@ AXG_API int axg_set_capacity(axg_ctx* c, uint64_t max_particles, uint32_t max_se
         c->n_B = 0;
     }
     c->max_particles = max_particles;
-    return AXG_OK;
+    return c->particles_allocated ? resolve_binning(c) : AXG_OK;  // AXG_BIN_AUTO depends on the capacity
 }
 
 AXG_API int axg_load_particles(axg_ctx* c, const float* x, const float* y, const float* z, const uint8_t* species,

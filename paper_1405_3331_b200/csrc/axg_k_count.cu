@@ -1,0 +1,192 @@
+// axg_k_count.cu -- P2 by cell counts (AXG_BIN_COUNT): the same outputs as the radix path (axg_k_sort.cu +
+// k_reorder) -- stable sorted permutation, sorted keys, reordered SoA, cell ranges -- computed as a counting sort
+// over the cells themselves (DESIGN.md §3 O4..O6, §6 "binning modes").
+//
+// Why it exists: on B200 the radix passes are issue-bound, not HBM-bound (profiles/), while the array of per-cell
+// counts (4 B x cells: 67 MB at C3) sits in the 126 MB L2.  So P1 counts particles per cell with one L2 atomic each,
+// and P2 is
+//   k_cell_scan  cell_lo = exclusive scan of cnt over the cells (single pass, decoupled look-back)  -> O6 for free
+//   k_place      slot[cell_lo[key] + arrival] = pre-sort index (| species << 30): cells are contiguous, the order
+//                INSIDE a cell is still the arbitrary arrival order of the atomics
+//   k_settle     every slot finds its rank among the members of its cell by pre-sort index (the order std::stable_sort
+//                gives equal keys, reading A-9), and the record moves to cell_lo + rank: O4 + O5.  Deterministic:
+//                nothing of the arrival order survives.  The first member of every cell re-zeroes cnt.
+// The paper's scheme sorts (cell hash, id) pairs and then finds cell starts; here the cell starts
+// come first and the sort is what is left inside a cell (mean occupancy of a non-empty cell is ~1.6 at C3).
+#include "axg_dev.cuh"
+
+namespace {
+
+// ---- exclusive scan of cnt[0 .. cells] --------------------------------------------------------------------------
+constexpr int SCAN_THREADS = 256;
+constexpr int SCAN_ITEMS = AXG_SCAN_TILE / SCAN_THREADS;  // 16 consecutive cells per thread: 4 x 128-bit
+constexpr int SCAN_WARPS = SCAN_THREADS / 32;
+
+__global__ void __launch_bounds__(SCAN_THREADS) k_cell_scan(const AxgParams p) {
+    __shared__ uint32_t s_warp[SCAN_WARPS];
+    __shared__ uint32_t s_tile, s_base;
+    AxgDev* dev = p.dev;
+    const uint32_t epoch = dev->epoch;
+    const uint32_t n_el = p.cells + 1u;  // cell_lo[cells] = n_live
+    const uint32_t n_tiles = (n_el + AXG_SCAN_TILE - 1) / AXG_SCAN_TILE;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+
+    while (true) {
+        __syncthreads();
+        if (tid == 0) s_tile = atomicAdd(&dev->ticket, 1u);
+        __syncthreads();
+        const uint32_t tile = s_tile;
+        if (tile >= n_tiles) break;
+        // the arrays are padded to a whole tile (zeros in cnt), so the vector accesses never leave them
+        const size_t at = (size_t)tile * AXG_SCAN_TILE + (size_t)tid * SCAN_ITEMS;
+        uint4 v[SCAN_ITEMS / 4];
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS / 4; ++k) v[k] = *reinterpret_cast<const uint4*>(p.cnt + at + 4 * k);
+        uint32_t tsum = 0u;
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS / 4; ++k) tsum += v[k].x + v[k].y + v[k].z + v[k].w;
+        uint32_t inc = tsum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t u = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += u;
+        }
+        if (lane == 31) s_warp[warp] = inc;
+        __syncthreads();
+        uint32_t woff = 0u, ttotal = 0u;
+#pragma unroll
+        for (int w = 0; w < SCAN_WARPS; ++w) {
+            const uint32_t c = s_warp[w];
+            woff += (w < warp) ? c : 0u;
+            ttotal += c;
+        }
+        if (warp == 0) {  // decoupled look-back, 32 predecessors per probe
+            uint32_t excl = 0u;
+            if (tile == 0) {
+                if (lane == 0) axg_st_state(p.scan_state + tile, axg_pack(epoch, AXG_FLAG_INCL, ttotal));
+            } else {
+                if (lane == 0) axg_st_state(p.scan_state + tile, axg_pack(epoch, AXG_FLAG_AGG, ttotal));
+                int q = (int)tile - 1 - lane;
+                while (true) {
+                    unsigned long long w;
+                    uint32_t f;
+                    do {
+                        w = (q >= 0) ? axg_ld_state(p.scan_state + q) : axg_pack(epoch, AXG_FLAG_INCL, 0u);
+                        f = axg_flag(w, epoch);
+                    } while (__any_sync(0xffffffffu, f == 0u));
+                    const uint32_t incl = __ballot_sync(0xffffffffu, f == (uint32_t)AXG_FLAG_INCL);
+                    uint32_t val = (uint32_t)w;
+                    if (incl) {
+                        const int firstincl = __ffs(incl) - 1;
+                        val = (lane <= firstincl) ? val : 0u;
+                        excl += __reduce_add_sync(0xffffffffu, val);
+                        break;
+                    }
+                    excl += __reduce_add_sync(0xffffffffu, val);
+                    q -= 32;
+                }
+                if (lane == 0) axg_st_state(p.scan_state + tile, axg_pack(epoch, AXG_FLAG_INCL, excl + ttotal));
+            }
+            if (lane == 0) s_base = excl;
+        }
+        __syncthreads();
+        uint32_t run = s_base + woff + inc - tsum;
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS / 4; ++k) {
+            uint4 o;
+            o.x = run; run += v[k].x;
+            o.y = run; run += v[k].y;
+            o.z = run; run += v[k].z;
+            o.w = run; run += v[k].w;
+            *reinterpret_cast<uint4*>(p.cell_lo + at + 4 * k) = o;
+        }
+    }
+    if (axg_last_block(dev) && tid == 0) {
+        dev->ticket = 0u;
+        dev->done = 0u;
+        dev->epoch = epoch + 1u;
+    }
+}
+
+// ---- slot[cell_lo[key] + arrival] = pre-sort index | species << 30 ----------------------------------------------
+constexpr int PLACE_THREADS = 256;
+
+__global__ void __launch_bounds__(PLACE_THREADS) k_place(const AxgParams p) {
+    const uint32_t n = p.dev->n_live;
+    uint32_t* __restrict__ slot = p.sidx[p.final_buf ^ 1];
+    const uint32_t* __restrict__ cell_lo = p.cell_lo;
+    const uint32_t n4 = n >> 2;
+    for (uint32_t g = blockIdx.x * PLACE_THREADS + threadIdx.x; g < n4; g += gridDim.x * PLACE_THREADS) {
+        const uint4 k = __ldg(reinterpret_cast<const uint4*>(p.key_pre) + g);
+        const uint4 a = __ldg(reinterpret_cast<const uint4*>(p.arrival) + g);
+        const uchar4 s = __ldg(reinterpret_cast<const uchar4*>(p.Bsp) + g);
+        const uint32_t o = g * 4u;
+        const uint32_t d0 = __ldg(cell_lo + k.x) + a.x, d1 = __ldg(cell_lo + k.y) + a.y,
+                       d2 = __ldg(cell_lo + k.z) + a.z, d3 = __ldg(cell_lo + k.w) + a.w;
+        slot[d0] = o | ((uint32_t)s.x << 30);
+        slot[d1] = (o + 1u) | ((uint32_t)s.y << 30);
+        slot[d2] = (o + 2u) | ((uint32_t)s.z << 30);
+        slot[d3] = (o + 3u) | ((uint32_t)s.w << 30);
+    }
+    if (blockIdx.x == 0 && threadIdx.x < (n & 3u)) {  // ragged tail
+        const uint32_t o = n4 * 4u + threadIdx.x;
+        slot[__ldg(cell_lo + p.key_pre[o]) + p.arrival[o]] = o | ((uint32_t)p.Bsp[o] << 30);
+    }
+}
+
+// ---- rank inside the cell by pre-sort index, then O5: A[cell_lo + rank] = B[index] -------------------------------
+constexpr int SETTLE_THREADS = 256;
+constexpr int SETTLE_ITEMS = 4;  // warp-striped: item i of lane l is slot base + 32 i + l, so every access of a
+                                 // warp instruction covers 32 neighbouring slots
+
+__global__ void __launch_bounds__(SETTLE_THREADS, 6) k_settle(const AxgParams p) {
+    const uint32_t n = p.dev->n_live;
+    const uint32_t* __restrict__ slot = p.sidx[p.final_buf ^ 1];
+    uint32_t* __restrict__ perm = p.sidx[p.final_buf];
+    uint32_t* __restrict__ keys = p.skey[p.final_buf];
+    const float4* __restrict__ rec = p.Brec;
+    const uint32_t* __restrict__ cell_lo = p.cell_lo;
+    const int lane = threadIdx.x & 31;
+    const uint32_t warps_total = (gridDim.x * SETTLE_THREADS) >> 5;
+    const uint32_t chunk = 32u * SETTLE_ITEMS;
+    for (uint32_t base = ((blockIdx.x * SETTLE_THREADS + threadIdx.x) >> 5) * chunk; base < n;
+         base += warps_total * chunk) {
+        uint32_t v[SETTLE_ITEMS];
+        float4 r[SETTLE_ITEMS];
+#pragma unroll
+        for (int i = 0; i < SETTLE_ITEMS; ++i) {
+            const uint32_t j = base + 32u * i + lane;
+            v[i] = (j < n) ? __ldg(slot + j) : 0u;
+        }
+#pragma unroll
+        for (int i = 0; i < SETTLE_ITEMS; ++i) {
+            const uint32_t j = base + 32u * i + lane;
+            r[i] = (j < n) ? __ldg(rec + (v[i] & AXG_IDX_MASK)) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+#pragma unroll
+        for (int i = 0; i < SETTLE_ITEMS; ++i) {
+            const uint32_t j = base + 32u * i + lane;
+            if (j >= n) continue;
+            const uint32_t idx = v[i] & AXG_IDX_MASK;
+            const uint32_t k = axg_cell_key(p, r[i].x, r[i].y, r[i].z);
+            const uint32_t lo = __ldg(cell_lo + k), hi = __ldg(cell_lo + k + 1u);
+            uint32_t rank = 0u;  // members of my cell with a smaller pre-sort index (reading A-9: ties keep that order)
+            for (uint32_t q = lo; q < hi; ++q) rank += ((__ldg(slot + q) & AXG_IDX_MASK) < idx) ? 1u : 0u;
+            const uint32_t dst = lo + rank;
+            p.A.x[dst] = r[i].x;
+            p.A.y[dst] = r[i].y;
+            p.A.z[dst] = r[i].z;
+            p.A.id[dst] = __float_as_uint(r[i].w);
+            p.A.species[dst] = (uint8_t)(v[i] >> 30);
+            keys[dst] = k;
+            perm[dst] = v[i];
+            if (rank == 0u) p.cnt[k] = 0u;  // cnt is all-zero again when the kernel ends
+        }
+    }
+}
+
+}  // namespace
+
+void axg_launch_cell_scan(const AxgParams& p, int grid, cudaStream_t s) { k_cell_scan<<<grid, SCAN_THREADS, 0, s>>>(p); }
+void axg_launch_place(const AxgParams& p, int grid, cudaStream_t s) { k_place<<<grid, PLACE_THREADS, 0, s>>>(p); }
+void axg_launch_settle(const AxgParams& p, int grid, cudaStream_t s) { k_settle<<<grid, SETTLE_THREADS, 0, s>>>(p); }

@@ -14,15 +14,16 @@ constexpr int DIFF_ITEMS = 8;
 constexpr int DIFF_TILE = DIFF_THREADS * DIFF_ITEMS;
 constexpr int DIFF_WARPS = DIFF_THREADS / 32;
 
-__device__ __forceinline__ uint32_t cell_key(const AxgParams& p, float x, float y, float z) {
-    // O3 / reading A-8: truncation of non-negative fp32, x fastest
-    return ((uint32_t)z * p.ny + (uint32_t)y) * p.nx + (uint32_t)x;
-}
-
-__device__ __forceinline__ void hist_add(uint32_t (*s_hist)[AXG_RADIX], int n_pass, uint32_t key) {
+// What P1 leaves for P2 besides the key: radix mode -- the digit histograms of every pass (shared memory, flushed
+// once per block); count mode -- the particle's arrival number in its cell, from one L2 atomic on cnt[key].
+__device__ __forceinline__ void tally(const AxgParams& p, uint32_t (*s_hist)[AXG_RADIX], uint32_t key, uint32_t o) {
+    if (p.bin_mode == AXG_BIN_COUNT_D) {
+        p.arrival[o] = atomicAdd(p.cnt + key, 1u);
+    } else {
 #pragma unroll
-    for (int q = 0; q < AXG_MAX_PASSES; ++q)
-        if (q < n_pass) atomicAdd(&s_hist[q][(key >> (8 * q)) & 0xffu], 1u);
+        for (int q = 0; q < AXG_MAX_PASSES; ++q)
+            if (q < p.n_pass) atomicAdd(&s_hist[q][(key >> (8 * q)) & 0xffu], 1u);
+    }
 }
 
 __global__ void __launch_bounds__(DIFF_THREADS, 3) k_diffuse(const AxgParams p) {
@@ -134,11 +135,11 @@ __global__ void __launch_bounds__(DIFF_THREADS, 3) k_diffuse(const AxgParams p) 
             const uint32_t b = __ballot_sync(0xffffffffu, a);
             if (a) {
                 const uint32_t o = out + __popc(b & lt);
-                const uint32_t key = cell_key(p, x[i], y[i], z[i]);
+                const uint32_t key = axg_cell_key(p, x[i], y[i], z[i]);
                 p.Brec[o] = make_float4(x[i], y[i], z[i], __uint_as_float(id[i]));
                 p.Bsp[o] = (uint8_t)((sp_pack[i >> 2] >> (8 * (i & 3))) & 0xffu);
                 p.key_pre[o] = key;
-                hist_add(s_hist, p.n_pass, key);
+                tally(p, s_hist, key, o);
             }
             out += __popc(b);
         }
@@ -165,11 +166,11 @@ __global__ void __launch_bounds__(256) k_rekey(const AxgParams p) {
     __syncthreads();
     for (uint32_t g = blockIdx.x * blockDim.x + threadIdx.x; g < n; g += gridDim.x * blockDim.x) {
         const float x = p.A.x[g], y = p.A.y[g], z = p.A.z[g];
-        const uint32_t key = cell_key(p, x, y, z);
+        const uint32_t key = axg_cell_key(p, x, y, z);
         p.Brec[g] = make_float4(x, y, z, __uint_as_float(p.A.id[g]));
         p.Bsp[g] = p.A.species[g];
         p.key_pre[g] = key;
-        hist_add(s_hist, p.n_pass, key);
+        tally(p, s_hist, key, g);
     }
     __syncthreads();
     for (int i = threadIdx.x; i < p.n_pass * AXG_RADIX; i += blockDim.x) {
@@ -204,11 +205,11 @@ __global__ void __launch_bounds__(EMIT_THREADS) k_emit(const AxgParams p, int do
             const uint32_t s = lo, j = e - p.src_emit_prefix[s];
             const AxgSourceDev sd = p.src[s];
             const uint32_t o = n_surv + e;
-            const uint32_t key = cell_key(p, sd.x, sd.y, sd.z);
+            const uint32_t key = axg_cell_key(p, sd.x, sd.y, sd.z);
             p.Brec[o] = make_float4(sd.x, sd.y, sd.z, __uint_as_float(next_id + p.src_id_prefix[s] + j));
             p.Bsp[o] = (uint8_t)(sd.species_polarity & 0xffu);
             p.key_pre[o] = key;
-            hist_add(s_hist, p.n_pass, key);
+            tally(p, s_hist, key, o);
         }
     }
     __syncthreads();

@@ -5,11 +5,19 @@ from oracle import axo
 from paper_1405_3331_b200 import workloads as W
 
 RTOL, ATOL = 1e-5, 1e-6   # BASELINE.json north_star: single-step fp32 positions, gradients, headings
+BINNING = None            # axg.BIN_RADIX / axg.BIN_COUNT: set by the parametrised fixture of the GPU tests
+
+
+def new_axg(axg_mod, *args):
+    g = axg_mod.Axg(*args)
+    if BINNING is not None:
+        g.set_binning(BINNING)
+    return g
 
 
 def make_pair(w, axg_mod, place=True):
     """The same workload applied to a CUDA context and an oracle context."""
-    g = axg_mod.Axg(w.grid, w.D, w.emission, w.radius, w.speed, w.noise, w.seed)
+    g = new_axg(axg_mod, w.grid, w.D, w.emission, w.radius, w.speed, w.noise, w.seed)
     o = axo.Oracle(w.grid, w.D, w.emission, w.radius, w.speed, w.noise, w.seed)
     W.apply(g, w, place=place)
     W.apply(o, w, place=place)

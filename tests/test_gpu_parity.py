@@ -10,17 +10,21 @@ import pytest
 from oracle import axo
 from paper_1405_3331_b200 import workloads as W
 
+import parity_util as pu
 from parity_util import (compare_binning, compare_cones, compare_presort, compare_sense, feed_gpu_presort_to_oracle,
                          load_same_particles, make_pair, pre_arrays)
 
 pytestmark = pytest.mark.gpu
 
 
-@pytest.fixture(scope="module")
-def axg():
+@pytest.fixture(scope="module", params=["radix", "count"])
+def axg(request):
+    """Every test runs under both binning modes (include/axg.h axg_set_binning): the results must be identical."""
     from paper_1405_3331_b200 import axg as m
     m.lib()
-    return m
+    pu.BINNING = m.BIN_RADIX if request.param == "radix" else m.BIN_COUNT
+    yield m
+    pu.BINNING = None
 
 
 def _chain(axg, w, n, seed, steps=2, n_species=2):
@@ -78,7 +82,7 @@ def test_chain_edge_sizes(axg, n):
 
 def test_empty_everything(axg):
     """No particles, no sources, no cones: a step is a no-op that still commits."""
-    g = axg.Axg((8, 8, 8), 0.5, 1, 2.0, 0.25, 0.1, 1)
+    g = pu.new_axg(axg, (8, 8, 8), 0.5, 1, 2.0, 0.25, 0.1, 1)
     g.step(3)
     c = g.counters()
     assert c["step"] == 3 and c["n_live"] == 0 and c["emitted"] == 0
@@ -90,7 +94,7 @@ def test_empty_everything(axg):
 def test_binning_only_on_given_positions(axg):
     """AXG_PHASE_BIN alone: copy + re-key + sort + reorder + ranges, against std::stable_sort binning."""
     for seed, grid, n in ((1, (256, 256, 256), 300_000), (2, (7, 5, 3), 20_000), (3, (1024, 1024, 256), 100_000)):
-        g = axg.Axg(grid, 0.5, 1, 2.0, 0.25, 0.1, seed)
+        g = pu.new_axg(axg, grid, 0.5, 1, 2.0, 0.25, 0.1, seed)
         o = axo.Oracle(grid, 0.5, 1, 2.0, 0.25, 0.1, seed)
         g.set_capacity(n + 16, 8)
         o.set_capacity(n + 16, 8)
@@ -107,7 +111,7 @@ def test_binning_only_on_given_positions(axg):
 def test_table1_of_the_paper_on_gpu(axg, golden_dir):
     """PAPER.md:267-276 Table 1 (reading A-17): 6 particles in cells 9 6 6 4 6 4 of a 16-cell row."""
     cells = np.array([9, 6, 6, 4, 6, 4])
-    g = axg.Axg((16, 1, 1), 0.5, 1, 2.0, 0.25, 0.1, 1)
+    g = pu.new_axg(axg, (16, 1, 1), 0.5, 1, 2.0, 0.25, 0.1, 1)
     x = cells.astype(np.float32) + 0.5
     zeros = np.zeros(6, np.float32)
     g.load_particles(x, zeros, zeros, np.zeros(6, np.uint8), np.arange(6, dtype=np.uint32), 6, 0)
@@ -140,7 +144,7 @@ def test_whole_steps_c1_from_empty(axg):
 
 
 def test_errors_and_capacity(axg):
-    g = axg.Axg((8, 8, 8), 0.5, 4, 2.0, 0.25, 0.1, 1)
+    g = pu.new_axg(axg, (8, 8, 8), 0.5, 4, 2.0, 0.25, 0.1, 1)
     g.set_capacity(10, 2)
     g.add_source(4, 4, 4, 0, 1, 4)
     with pytest.raises(axg.AxgError) as e:
