@@ -192,9 +192,8 @@ int alloc_particles(axg_ctx* c, uint64_t cap, AxgParams& P, std::vector<void*>& 
     const size_t sizes[] = {n * 4, n * 4, n * 4, n, n * 4,  // A (SoA)
                             n * 16, n,                      // Brec, Bsp
                             n * 4, n * 4, n * 4, n * 4, n * 4,  // key_pre, skey[2], sidx[2]
-                            diff_tiles * 8, sort_tiles * AXG_RADIX * 8,
-                            n * 4};                         // arrival
-    constexpr int NB = 15;
+                            diff_tiles * 8, sort_tiles * AXG_RADIX * 8};
+    constexpr int NB = 14;
     void* ptr[NB];
     for (int i = 0; i < NB; ++i) {
         ptr[i] = dev_alloc(c, sizes[i]);
@@ -213,7 +212,6 @@ int alloc_particles(axg_ctx* c, uint64_t cap, AxgParams& P, std::vector<void*>& 
     P.sidx[0] = (uint32_t*)ptr[10]; P.sidx[1] = (uint32_t*)ptr[11];
     P.tile_state = (unsigned long long*)ptr[12];
     P.sort_state = (unsigned long long*)ptr[13];
-    P.arrival = (uint32_t*)ptr[14];
     P.capacity = (uint32_t)cap;
     // look-back words must not alias a live epoch: zero them (epoch 0 words with flag 0 = not ready)
     CU(c, cudaMemsetAsync(ptr[12], 0, sizes[12], c->stream));
@@ -358,10 +356,8 @@ int enqueue_phases(axg_ctx* c, uint32_t mask, Prof& prof) {
     if (mask & AXG_PHASE_DIFFUSE) {
         zero_cnt_if_dirty();
         prof.mark(AXG_K_DIFFUSE);
-        axg_launch_diffuse(P, N_SM * 3, s);
-        prof.mark(AXG_K_EMIT);
-        axg_launch_emit(P, 1, s);
-        launches += 2;
+        axg_launch_diffuse(P, N_SM * 3, s);  // its last block emits and closes P1
+        launches += 1;
         c->cnt_dirty = count_mode;
     }
     if (mask & AXG_PHASE_BIN) {

@@ -69,6 +69,7 @@ __global__ void __launch_bounds__(256) k_sense(const AxgParams p) {
 __global__ void __launch_bounds__(128) k_advance(const AxgParams p) {
     AxgDev* dev = p.dev;
     const uint32_t t = dev->step;
+    const AxgRoundKeys rk = axg_round_keys(p.seed_lo, p.seed_hi);
     for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < p.n_cones; c += gridDim.x * blockDim.x) {
         if (p.cone_state[c] != 0) continue;
         long long G[3] = {0, 0, 0};
@@ -93,7 +94,7 @@ __global__ void __launch_bounds__(128) k_advance(const AxgParams p) {
             g[0] = __fdiv_rn(gx, len); g[1] = __fdiv_rn(gy, len); g[2] = __fdiv_rn(gz, len);
         }
         float xi[3];
-        axg_normals3(c, t, 1u, p.seed_lo, p.seed_hi, xi[0], xi[1], xi[2]);  // stream 1 = cone noise (A-2)
+        axg_normals3(c, t, 1u, rk, xi[0], xi[1], xi[2]);  // stream 1 = cone noise (A-2)
         float v[3];
 #pragma unroll
         for (int a = 0; a < 3; ++a) v[a] = __fadd_rn(g[a], __fmul_rn(p.noise, xi[a]));  // reading A-15

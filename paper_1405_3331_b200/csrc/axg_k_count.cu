@@ -5,12 +5,13 @@
 // Why it exists: on B200 the radix passes are issue-bound, not HBM-bound (profiles/), while the array of per-cell
 // counts (4 B x cells: 67 MB at C3) sits in the 126 MB L2.  So P1 counts particles per cell with one L2 atomic each,
 // and P2 is
-//   k_cell_scan  cell_lo = exclusive scan of cnt over the cells (single pass, decoupled look-back)  -> O6 for free
-//   k_place      slot[cell_lo[key] + arrival] = pre-sort index (| species << 30): cells are contiguous, the order
-//                INSIDE a cell is still the arbitrary arrival order of the atomics
+//   k_cell_scan  cell_lo = exclusive scan of cnt over the cells (single pass, decoupled look-back)  -> O6 for free;
+//                cnt is re-zeroed on the way
+//   k_place      slot[atomicAdd(cursor of the cell)] = pre-sort index (| species << 30): cells are contiguous, the
+//                order INSIDE a cell is the arbitrary order of the atomics
 //   k_settle     every slot finds its rank among the members of its cell by pre-sort index (the order std::stable_sort
 //                gives equal keys, reading A-9), and the record moves to cell_lo + rank: O4 + O5.  Deterministic:
-//                nothing of the arrival order survives.  The first member of every cell re-zeroes cnt.
+//                nothing of the arrival order survives.
 // The paper's scheme sorts (cell hash, id) pairs and then finds cell starts; here the cell starts
 // come first and the sort is what is left inside a cell (mean occupancy of a non-empty cell is ~1.6 at C3).
 #include "axg_dev.cuh"
@@ -18,8 +19,8 @@
 namespace {
 
 // ---- exclusive scan of cnt[0 .. cells] --------------------------------------------------------------------------
-constexpr int SCAN_THREADS = 256;
-constexpr int SCAN_ITEMS = AXG_SCAN_TILE / SCAN_THREADS;  // 16 consecutive cells per thread: 4 x 128-bit
+constexpr int SCAN_THREADS = 512;
+constexpr int SCAN_ITEMS = AXG_SCAN_TILE / SCAN_THREADS;  // 32 consecutive cells per thread: 8 x 128-bit
 constexpr int SCAN_WARPS = SCAN_THREADS / 32;
 
 __global__ void __launch_bounds__(SCAN_THREADS) k_cell_scan(const AxgParams p) {
@@ -37,20 +38,28 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_cell_scan(const AxgParams p) {
         __syncthreads();
         const uint32_t tile = s_tile;
         if (tile >= n_tiles) break;
-        // the arrays are padded to a whole tile (zeros in cnt), so the vector accesses never leave them
-        const size_t at = (size_t)tile * AXG_SCAN_TILE + (size_t)tid * SCAN_ITEMS;
+        // the arrays are padded to a whole tile (zeros in cnt), so the vector accesses never leave them.  Every warp
+        // owns 1024 consecutive cells; chunk c of a lane is the 4 cells at (32 c + lane) * 4: each load and store
+        // instruction of the warp covers 512 contiguous bytes.
+        const size_t at4 = ((size_t)tile * AXG_SCAN_TILE + (size_t)warp * (32 * SCAN_ITEMS)) / 4 + lane;
         uint4 v[SCAN_ITEMS / 4];
 #pragma unroll
-        for (int k = 0; k < SCAN_ITEMS / 4; ++k) v[k] = *reinterpret_cast<const uint4*>(p.cnt + at + 4 * k);
-        uint32_t tsum = 0u;
+        for (int k = 0; k < SCAN_ITEMS / 4; ++k) v[k] = reinterpret_cast<const uint4*>(p.cnt)[at4 + 32 * k];
+        uint32_t pre[SCAN_ITEMS / 4];  // particles before my 4 cells of chunk k, inside the warp's segment
+        uint32_t carry = 0u;
 #pragma unroll
-        for (int k = 0; k < SCAN_ITEMS / 4; ++k) tsum += v[k].x + v[k].y + v[k].z + v[k].w;
-        uint32_t inc = tsum;
+        for (int k = 0; k < SCAN_ITEMS / 4; ++k) {
+            const uint32_t mine = v[k].x + v[k].y + v[k].z + v[k].w;
+            uint32_t incl = mine;
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t u = __shfl_up_sync(0xffffffffu, inc, o);
-            if (lane >= o) inc += u;
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t u = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += u;
+            }
+            pre[k] = carry + incl - mine;
+            carry += __shfl_sync(0xffffffffu, incl, 31);
         }
+        const uint32_t inc = carry;  // the warp's total, in every lane
         if (lane == 31) s_warp[warp] = inc;
         __syncthreads();
         uint32_t woff = 0u, ttotal = 0u;
@@ -90,15 +99,22 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_cell_scan(const AxgParams p) {
             if (lane == 0) s_base = excl;
         }
         __syncthreads();
-        uint32_t run = s_base + woff + inc - tsum;
+        // cnt is counted SHIFTED by one cell (P1 adds to cnt[key + 1]), so this plain exclusive scan leaves in
+        // cell_lo[j] the particles below cell j - 1 = the cursor of cell j - 1.  k_place bumps cell_lo[key + 1] once per
+        // particle of cell `key`, which turns the entry into the particles below cell key + 1: after k_place the array
+        // is the exclusive scan of the true counts, with no second array and no gather.  cnt is re-zeroed on the way.
+        const uint32_t wbase = s_base + woff;
+        const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
 #pragma unroll
         for (int k = 0; k < SCAN_ITEMS / 4; ++k) {
+            uint32_t run = wbase + pre[k];
             uint4 o;
             o.x = run; run += v[k].x;
             o.y = run; run += v[k].y;
             o.z = run; run += v[k].z;
-            o.w = run; run += v[k].w;
-            *reinterpret_cast<uint4*>(p.cell_lo + at + 4 * k) = o;
+            o.w = run;
+            reinterpret_cast<uint4*>(p.cell_lo)[at4 + 32 * k] = o;
+            reinterpret_cast<uint4*>(p.cnt)[at4 + 32 * k] = zero;
         }
     }
     if (axg_last_block(dev) && tid == 0) {
@@ -108,21 +124,26 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_cell_scan(const AxgParams p) {
     }
 }
 
-// ---- slot[cell_lo[key] + arrival] = pre-sort index | species << 30 ----------------------------------------------
+// ---- slot[cursor(key)++] = pre-sort index | species << 30 ---------------------------------------------------------
 constexpr int PLACE_THREADS = 256;
+
+// the cursor of cell k lives in cell_lo[k + 1] (see k_cell_scan): one L2 atomic, no other access to the cell arrays
+__device__ __forceinline__ uint32_t take_slot(uint32_t* __restrict__ cell_lo, uint32_t k) {
+    return atomicAdd(cell_lo + k + 1u, 1u);
+}
 
 __global__ void __launch_bounds__(PLACE_THREADS) k_place(const AxgParams p) {
     const uint32_t n = p.dev->n_live;
     uint32_t* __restrict__ slot = p.sidx[p.final_buf ^ 1];
-    const uint32_t* __restrict__ cell_lo = p.cell_lo;
+    uint32_t* __restrict__ cell_lo = p.cell_lo;
     const uint32_t n4 = n >> 2;
     for (uint32_t g = blockIdx.x * PLACE_THREADS + threadIdx.x; g < n4; g += gridDim.x * PLACE_THREADS) {
         const uint4 k = __ldg(reinterpret_cast<const uint4*>(p.key_pre) + g);
-        const uint4 a = __ldg(reinterpret_cast<const uint4*>(p.arrival) + g);
         const uchar4 s = __ldg(reinterpret_cast<const uchar4*>(p.Bsp) + g);
         const uint32_t o = g * 4u;
-        const uint32_t d0 = __ldg(cell_lo + k.x) + a.x, d1 = __ldg(cell_lo + k.y) + a.y,
-                       d2 = __ldg(cell_lo + k.z) + a.z, d3 = __ldg(cell_lo + k.w) + a.w;
+        // bumping the cursor hands out the slots of the cell in the arbitrary order of the atomics
+        const uint32_t d0 = take_slot(cell_lo, k.x), d1 = take_slot(cell_lo, k.y), d2 = take_slot(cell_lo, k.z),
+                       d3 = take_slot(cell_lo, k.w);
         slot[d0] = o | ((uint32_t)s.x << 30);
         slot[d1] = (o + 1u) | ((uint32_t)s.y << 30);
         slot[d2] = (o + 2u) | ((uint32_t)s.z << 30);
@@ -130,7 +151,7 @@ __global__ void __launch_bounds__(PLACE_THREADS) k_place(const AxgParams p) {
     }
     if (blockIdx.x == 0 && threadIdx.x < (n & 3u)) {  // ragged tail
         const uint32_t o = n4 * 4u + threadIdx.x;
-        slot[__ldg(cell_lo + p.key_pre[o]) + p.arrival[o]] = o | ((uint32_t)p.Bsp[o] << 30);
+        slot[take_slot(cell_lo, p.key_pre[o])] = o | ((uint32_t)p.Bsp[o] << 30);
     }
 }
 
@@ -180,7 +201,6 @@ __global__ void __launch_bounds__(SETTLE_THREADS, 6) k_settle(const AxgParams p)
             p.A.species[dst] = (uint8_t)(v[i] >> 30);
             keys[dst] = k;
             perm[dst] = v[i];
-            if (rank == 0u) p.cnt[k] = 0u;  // cnt is all-zero again when the kernel ends
         }
     }
 }

@@ -2,7 +2,8 @@
 //   k_diffuse  Brownian step of every live particle (Philox4x32-10 keyed on (seed, id, t) -> Box-Muller -> fma),
 //              absorbing-boundary test, ORDER-PRESERVING compaction (warp ballot/popc ranks, block scan, one
 //              decoupled look-back word per tile), cell key, per-pass digit histograms for the radix sort.
-//   k_emit     newborns of every owned source appended after the survivors, counters, histogram scan.
+//   emit_and_close  newborns of every owned source appended after the survivors, counters, histogram scan: run by
+//              the last block of k_diffuse to finish (k_emit = the same after k_rekey, harness path).
 //   k_rekey    harness path (AXG_PHASE_BIN without AXG_PHASE_DIFFUSE): copy A -> B and key it.
 // Paper: integration kernel + calculateHash, PAPER.md:263 (§3.5); particles "generated ... and die".
 #include "axg_dev.cuh"
@@ -15,14 +16,87 @@ constexpr int DIFF_TILE = DIFF_THREADS * DIFF_ITEMS;
 constexpr int DIFF_WARPS = DIFF_THREADS / 32;
 
 // What P1 leaves for P2 besides the key: radix mode -- the digit histograms of every pass (shared memory, flushed
-// once per block); count mode -- the particle's arrival number in its cell, from one L2 atomic on cnt[key].
-__device__ __forceinline__ void tally(const AxgParams& p, uint32_t (*s_hist)[AXG_RADIX], uint32_t key, uint32_t o) {
+// once per block); count mode -- one more particle in cnt[key] (L2 reduction, no return value).
+__device__ __forceinline__ void tally(const AxgParams& p, uint32_t (*s_hist)[AXG_RADIX], uint32_t key) {
     if (p.bin_mode == AXG_BIN_COUNT_D) {
-        p.arrival[o] = atomicAdd(p.cnt + key, 1u);
+        atomicAdd(p.cnt + key + 1u, 1u);  // shifted by one cell (see k_cell_scan); result unused: a fire-and-forget RED
     } else {
 #pragma unroll
         for (int q = 0; q < AXG_MAX_PASSES; ++q)
             if (q < p.n_pass) atomicAdd(&s_hist[q][(key >> (8 * q)) & 0xffu], 1u);
+    }
+}
+
+// O2: newborns (reading A-5: exactly at the source, not moved in their birth step; A-6: after the survivors, in
+// (source, j) order), counters, and -- radix mode -- the exclusive scans of the digit histograms that the sort passes
+// start from.  Run by ONE block: the last block of k_diffuse to finish, or k_emit (do_emit == 0: harness path after
+// k_rekey).  s_hist must hold AXG_MAX_PASSES x AXG_RADIX words; its contents are overwritten.
+__device__ void emit_and_close(const AxgParams& p, int do_emit, uint32_t (*s_hist)[AXG_RADIX]) {
+    __shared__ uint32_t s_scan[AXG_RADIX / 32];
+    AxgDev* dev = p.dev;
+    const int tid = threadIdx.x, nthr = blockDim.x;
+    const uint32_t n_in = dev->n_live;
+    const uint32_t n_surv = do_emit ? (n_in ? dev->n_surv : 0u) : n_in;
+    const uint32_t next_id = dev->next_id;
+    const bool fits = (unsigned long long)n_surv + p.e_owned <= (unsigned long long)p.capacity;
+    __syncthreads();
+    for (int i = tid; i < AXG_MAX_PASSES * AXG_RADIX; i += nthr) (&s_hist[0][0])[i] = 0u;
+    __syncthreads();
+    if (do_emit && fits) {
+        for (uint32_t e = tid; e < p.e_owned; e += nthr) {
+            // source s with src_emit_prefix[s] <= e < src_emit_prefix[s+1]
+            uint32_t lo = 0u, hi = p.n_src;
+            while (hi - lo > 1u) {
+                const uint32_t mid = (lo + hi) >> 1;
+                if (p.src_emit_prefix[mid] <= e) lo = mid; else hi = mid;
+            }
+            const uint32_t s = lo, j = e - p.src_emit_prefix[s];
+            const AxgSourceDev sd = p.src[s];
+            const uint32_t o = n_surv + e;
+            const uint32_t key = axg_cell_key(p, sd.x, sd.y, sd.z);
+            p.Brec[o] = make_float4(sd.x, sd.y, sd.z, __uint_as_float(next_id + p.src_id_prefix[s] + j));
+            p.Bsp[o] = (uint8_t)(sd.species_polarity & 0xffu);
+            p.key_pre[o] = key;
+            if (p.bin_mode != AXG_BIN_COUNT_D) {
+                tally(p, s_hist, key);
+            } else if (j == 0u) {  // all newborns of a source share its cell: one reduction per source, not per particle
+                atomicAdd(p.cnt + key + 1u, p.src_emit_prefix[s + 1] - p.src_emit_prefix[s]);
+            }
+        }
+    }
+    __syncthreads();
+    if (p.bin_mode != AXG_BIN_COUNT_D) {
+        // total histogram -> exclusive scan per pass; needs >= 256 threads (one digit each)
+        for (int q = 0; q < p.n_pass; ++q) {
+            const int d = tid, lane = tid & 31, wq = tid >> 5;
+            uint32_t c = 0u, inc = 0u;
+            if (d < AXG_RADIX) {
+                c = dev->hist[q][d] + s_hist[q][d];
+                inc = c;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o);
+                    if (lane >= o) inc += v;
+                }
+                if (lane == 31) s_scan[wq] = inc;
+            }
+            __syncthreads();
+            if (d < AXG_RADIX) {
+                uint32_t off = 0u;
+                for (int w = 0; w < wq; ++w) off += s_scan[w];
+                dev->base[q][d] = off + inc - c;
+                dev->hist[q][d] = 0u;
+            }
+            __syncthreads();
+        }
+    }
+    if (tid == 0 && do_emit) {
+        if (!fits) dev->err |= 1u;
+        dev->n_live = fits ? n_surv + p.e_owned : n_surv;
+        dev->next_id = next_id + p.e_total;
+        dev->emitted += fits ? p.e_owned : 0u;
+        dev->absorbed += n_in - n_surv;
+        dev->particle_steps += n_in;
     }
 }
 
@@ -36,6 +110,7 @@ __global__ void __launch_bounds__(DIFF_THREADS, 3) k_diffuse(const AxgParams p) 
     const uint32_t n_tiles = (n_in + DIFF_TILE - 1) / DIFF_TILE;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t lt = axg_lanemask_lt();
+    const AxgRoundKeys rk = axg_round_keys(p.seed_lo, p.seed_hi);
 
     for (int i = tid; i < AXG_MAX_PASSES * AXG_RADIX; i += DIFF_THREADS) (&s_hist[0][0])[i] = 0u;
 
@@ -71,7 +146,7 @@ __global__ void __launch_bounds__(DIFF_THREADS, 3) k_diffuse(const AxgParams p) 
         for (int i = 0; i < DIFF_ITEMS; ++i) {
             const bool v = (first + i * 32) < n_in;
             float z0, z1, z2;
-            axg_normals3(id[i], t, 0u, p.seed_lo, p.seed_hi, z0, z1, z2);
+            axg_normals3(id[i], t, 0u, rk, z0, z1, z2);
             x[i] = fmaf(p.sigma, z0, x[i]);
             y[i] = fmaf(p.sigma, z1, y[i]);
             z[i] = fmaf(p.sigma, z2, z[i]);
@@ -139,7 +214,7 @@ __global__ void __launch_bounds__(DIFF_THREADS, 3) k_diffuse(const AxgParams p) 
                 p.Brec[o] = make_float4(x[i], y[i], z[i], __uint_as_float(id[i]));
                 p.Bsp[o] = (uint8_t)((sp_pack[i >> 2] >> (8 * (i & 3))) & 0xffu);
                 p.key_pre[o] = key;
-                tally(p, s_hist, key, o);
+                tally(p, s_hist, key);
             }
             out += __popc(b);
         }
@@ -150,10 +225,14 @@ __global__ void __launch_bounds__(DIFF_THREADS, 3) k_diffuse(const AxgParams p) 
         const uint32_t c = (&s_hist[0][0])[i];
         if (c) atomicAdd(&dev->hist[0][0] + i, c);
     }
-    if (axg_last_block(dev) && tid == 0) {
-        dev->ticket = 0u;
-        dev->done = 0u;
-        dev->epoch = epoch + 1u;
+    if (axg_last_block(dev)) {  // every block's survivors, keys and histogram flushes are visible here
+        if (tid == 0) {
+            dev->ticket = 0u;
+            dev->done = 0u;
+            dev->epoch = epoch + 1u;
+        }
+        __threadfence();
+        emit_and_close(p, 1, s_hist);
     }
 }
 
@@ -170,7 +249,7 @@ __global__ void __launch_bounds__(256) k_rekey(const AxgParams p) {
         p.Brec[g] = make_float4(x, y, z, __uint_as_float(p.A.id[g]));
         p.Bsp[g] = p.A.species[g];
         p.key_pre[g] = key;
-        tally(p, s_hist, key, g);
+        tally(p, s_hist, key);
     }
     __syncthreads();
     for (int i = threadIdx.x; i < p.n_pass * AXG_RADIX; i += blockDim.x) {
@@ -179,66 +258,10 @@ __global__ void __launch_bounds__(256) k_rekey(const AxgParams p) {
     }
 }
 
-// O2: newborns (reading A-5: exactly at the source, not moved in their birth step; A-6: after the survivors, in
-// (source, j) order), counters, and the exclusive scans of the digit histograms that the sort passes start from.
-// One block.  do_emit == 0 is the harness path after k_rekey.
-constexpr int EMIT_THREADS = 1024;
+constexpr int EMIT_THREADS = 256;
 __global__ void __launch_bounds__(EMIT_THREADS) k_emit(const AxgParams p, int do_emit) {
     __shared__ uint32_t s_hist[AXG_MAX_PASSES][AXG_RADIX];
-    __shared__ uint32_t s_scan[AXG_MAX_PASSES][AXG_RADIX / 32];
-    AxgDev* dev = p.dev;
-    const int tid = threadIdx.x;
-    const uint32_t n_in = dev->n_live;
-    const uint32_t n_surv = do_emit ? (n_in ? dev->n_surv : 0u) : n_in;
-    const uint32_t next_id = dev->next_id;
-    const bool fits = (unsigned long long)n_surv + p.e_owned <= (unsigned long long)p.capacity;
-    for (int i = tid; i < AXG_MAX_PASSES * AXG_RADIX; i += EMIT_THREADS) (&s_hist[0][0])[i] = 0u;
-    __syncthreads();
-    if (do_emit && fits) {
-        for (uint32_t e = tid; e < p.e_owned; e += EMIT_THREADS) {
-            // source s with src_emit_prefix[s] <= e < src_emit_prefix[s+1]
-            uint32_t lo = 0u, hi = p.n_src;
-            while (hi - lo > 1u) {
-                const uint32_t mid = (lo + hi) >> 1;
-                if (p.src_emit_prefix[mid] <= e) lo = mid; else hi = mid;
-            }
-            const uint32_t s = lo, j = e - p.src_emit_prefix[s];
-            const AxgSourceDev sd = p.src[s];
-            const uint32_t o = n_surv + e;
-            const uint32_t key = axg_cell_key(p, sd.x, sd.y, sd.z);
-            p.Brec[o] = make_float4(sd.x, sd.y, sd.z, __uint_as_float(next_id + p.src_id_prefix[s] + j));
-            p.Bsp[o] = (uint8_t)(sd.species_polarity & 0xffu);
-            p.key_pre[o] = key;
-            tally(p, s_hist, key, o);
-        }
-    }
-    __syncthreads();
-    // total histogram -> exclusive scan per pass (1024 threads = 4 passes x 256 digits)
-    const int q = tid >> 8, d = tid & 255, lane = tid & 31, wq = d >> 5;
-    uint32_t c = 0u;
-    if (q < p.n_pass) c = dev->hist[q][d] + s_hist[q][d];
-    uint32_t inc = c;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o);
-        if (lane >= o) inc += v;
-    }
-    if (lane == 31) s_scan[q][wq] = inc;
-    __syncthreads();
-    uint32_t off = 0u;
-    for (int w = 0; w < wq; ++w) off += s_scan[q][w];
-    dev->base[q][d] = off + inc - c;
-    dev->hist[q][d] = 0u;
-    if (tid == 0) {
-        if (do_emit) {
-            if (!fits) dev->err |= 1u;
-            dev->n_live = fits ? n_surv + p.e_owned : n_surv;
-            dev->next_id = next_id + p.e_total;
-            dev->emitted += fits ? p.e_owned : 0u;
-            dev->absorbed += n_in - n_surv;
-            dev->particle_steps += n_in;
-        }
-    }
+    emit_and_close(p, do_emit, s_hist);
 }
 
 }  // namespace
