@@ -87,12 +87,18 @@ def compare_binning(g, o):
         assert np.array_equal(a.view(np.uint32), b.view(np.uint32)), f
 
 
-def compare_sense(g, o, active_only=None):
-    gc, oc = g.read_state("CONE_COUNTS"), o.read_state("CONE_COUNTS")
-    gm, om = g.read_state("CONE_MOMENT"), o.read_state("CONE_MOMENT")
+def compare_sense(g, o, active_only=False):
+    """active_only: the fields hold the sums of the last P3 in which a cone was ACTIVE; an oracle that was handed a
+    snapshot has no history for the frozen ones, so only the active cones are comparable."""
+    gc, oc = g.read_state("CONE_COUNTS").reshape(-1, 4), o.read_state("CONE_COUNTS").reshape(-1, 4)
+    gm, om = g.read_state("CONE_MOMENT").reshape(-1, 12), o.read_state("CONE_MOMENT").reshape(-1, 12)
+    gg, og = g.read_state("CONE_GRADIENT").reshape(-1, 3), o.read_state("CONE_GRADIENT").reshape(-1, 3)
+    if active_only:
+        act = o.read_state("CONE_STATE") == 0
+        assert np.array_equal(act, g.read_state("CONE_STATE") == 0)
+        gc, oc, gm, om, gg, og = gc[act], oc[act], gm[act], om[act], gg[act], og[act]
     assert np.array_equal(gc, oc), "per-cone counts differ"
     assert np.array_equal(gm, om), "per-cone moments differ"
-    gg, og = g.read_state("CONE_GRADIENT"), o.read_state("CONE_GRADIENT")
     assert close(gg, og).all()
 
 

@@ -1,0 +1,91 @@
+"""Multi-step GPU-vs-oracle agreement (BASELINE.json north_star: "multi-step runs must agree statistically: MSD, counts
+and the radial profile within 1 %, and cone-to-target arrival fraction within 2 percentage points over 8 seeds").
+
+Both sides draw the same Philox streams, so they differ only through ulp-level Box-Muller differences and the rare
+boundary flips of reading A-19; the bars below are NS's, not tighter ones."""
+import numpy as np
+import pytest
+
+from oracle import axo
+from paper_1405_3331_b200 import workloads as W
+
+import parity_util as pu
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", params=["radix", "count"])
+def axg(request):
+    from paper_1405_3331_b200 import axg as m
+    m.lib()
+    pu.BINNING = m.BIN_RADIX if request.param == "radix" else m.BIN_COUNT
+    yield m
+    pu.BINNING = None
+
+
+def test_free_space_msd(axg):
+    """T4 on both sides: a burst at the centre of a 128^3 box, nothing reaches a wall in 20 steps: MSD = 6 D t."""
+    n, D, grid = 200_000, 0.5, (128, 128, 128)
+    c = np.full(n, 64.25, np.float32)
+    ids = np.arange(n, dtype=np.uint32)
+    sims = [pu.new_axg(axg, grid, D, 1, 2.0, 0.25, 0.1, 77), axo.Oracle(grid, D, 1, 2.0, 0.25, 0.1, 77)]
+    msd = []
+    for s in sims:
+        s.set_capacity(n + 8, 4)
+        s.load_particles(c, c, c, np.zeros(n, np.uint8), ids, next_id=n, step=0)
+        out = []
+        for t in (5, 20):
+            s.step(t - (0 if not out else 5))
+            x, y, z = (s.read_state("PART_" + k).astype(np.float64) for k in "XYZ")
+            assert len(x) == n
+            out.append(((x - 64.25) ** 2 + (y - 64.25) ** 2 + (z - 64.25) ** 2).mean())
+        msd.append(out)
+        s.close()
+    for t, g, o in zip((5, 20), msd[0], msd[1]):
+        assert abs(g / (6 * D * t) - 1) < 0.01, (t, g)
+        assert abs(g / o - 1) < 0.01, (t, g, o)
+
+
+def test_counts_and_axis_profile(axg):
+    """A source in an absorbing 32^3 box, 400 steps from empty: n_live(t), emitted - absorbed, and the z profile."""
+    grid = (32, 32, 32)
+    g = pu.new_axg(axg, grid, 0.5, 400, 2.0, 0.25, 0.1, 5)
+    o = axo.Oracle(grid, 0.5, 400, 2.0, 0.25, 0.1, 5)
+    live = [[], []]
+    prof = [np.zeros(32), np.zeros(32)]
+    for i, s in enumerate((g, o)):
+        s.set_capacity(200_000, 4)
+        s.add_source(16.5, 16.5, 12.5, 0, 1, 400)
+        for k in range(40):
+            s.step(10)
+            c = s.counters()
+            assert c["n_live"] == c["emitted"] - c["absorbed"]          # T3, every 10 steps
+            live[i].append(c["n_live"])
+            if k >= 20:
+                prof[i] += np.bincount(s.read_state("PART_Z").astype(np.int64), minlength=32)
+        s.close()
+    live = np.array(live, dtype=np.float64)
+    assert np.all(np.abs(live[0] / live[1] - 1) < 0.01), np.abs(live[0] / live[1] - 1).max()
+    big = prof[1] > 0.01 * prof[1].sum()
+    assert np.all(np.abs(prof[0][big] / prof[1][big] - 1) < 0.01)
+
+
+def test_arrival_fraction_over_8_seeds(axg):
+    """T12 (parity unpinned in absolute terms): 32 cones under one source, 8 seeds; fractions within 2 points."""
+    grid = (32, 32, 32)
+    arrived = [0, 0]
+    total = 0
+    for seed in range(8):
+        rng = np.random.default_rng(100 + seed)
+        cones = np.stack([rng.uniform(8, 24, 32), rng.uniform(8, 24, 32), np.full(32, 0.5)], 1).astype(np.float32)
+        sims = (pu.new_axg(axg, grid, 0.5, 256, 2.0, 0.25, 0.1, seed), axo.Oracle(grid, 0.5, 256, 2.0, 0.25, 0.1, seed))
+        for i, s in enumerate(sims):
+            s.set_capacity(200_000, 520)
+            s.add_source(16.0, 16.0, 26.0, 0, 1, 256)
+            s.place_neurons(cones, None)
+            s.step(500)
+            arrived[i] += s.counters()["arrived"]
+            s.close()
+        total += 32
+    fg, fo = arrived[0] / total, arrived[1] / total
+    assert abs(fg - fo) <= 0.02, (fg, fo)

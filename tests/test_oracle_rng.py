@@ -146,3 +146,13 @@ def test_T2_uniform_and_normal_moments():
     _, _, z_s1 = axo.normals(12345, 0, 1000, 3, 1)
     _, _, z_t4 = axo.normals(12345, 0, 1000, 4, 0)
     assert not np.array_equal(z_s1, z[:1000]) and not np.array_equal(z_t4, z[:1000])
+
+
+def test_uniform_built_without_int_to_float_is_the_same_number():
+    """Reading A-3: the kernel forms u as asfloat(0x3f800000 | r >> 9) - (1 - 2^-24); that must be THE value
+    ((r >> 9) * 2 + 1) * 2^-24 for every 23-bit mantissa (all 2^23 of them), else both sides would draw differently."""
+    m = np.arange(1 << 23, dtype=np.uint32)
+    spec = ((m << np.uint32(1)) | np.uint32(1)).astype(np.float32) * np.float32(2.0 ** -24)
+    built = (m | np.uint32(0x3F800000)).view(np.float32) + np.float32(-float.fromhex("0x1.fffffep-1"))
+    assert built.dtype == np.float32 and np.array_equal(spec.view(np.uint32), built.view(np.uint32))
+    assert spec.min() == np.float32(2.0 ** -24) and spec.max() == np.float32(1 - 2.0 ** -24)
