@@ -390,12 +390,14 @@ int enqueue_phases(axg_ctx* c, uint32_t mask, Prof& prof) {
         axg_launch_sense(P, s);
         launches += 1;
     }
+    bool committed = false;
     if ((mask & AXG_PHASE_ADVANCE) && P.n_cones) {
         prof.mark(AXG_K_ADVANCE);
-        axg_launch_advance(P, s);
+        committed = (mask & AXG_PHASE_COMMIT) != 0;  // O10 rides in the last block of k_advance
+        axg_launch_advance(P, committed ? 1 : 0, s);
         launches += 1;
     }
-    if (mask & AXG_PHASE_COMMIT) {
+    if ((mask & AXG_PHASE_COMMIT) && !committed) {
         prof.mark(AXG_K_COMMIT);
         axg_launch_commit(P, s);
         launches += 1;

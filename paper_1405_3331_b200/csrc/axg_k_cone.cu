@@ -66,7 +66,8 @@ __global__ void __launch_bounds__(256) k_sense(const AxgParams p) {
 // ---- P4 + P5: one thread per cone ------------------------------------------------------------------------------
 // Every fp32 operation that the specification fixes is written with the explicit round-to-nearest intrinsics so
 // that nvcc cannot contract it into an fma (reading A-22); only the normals may differ by an ulp.
-__global__ void __launch_bounds__(128) k_advance(const AxgParams p) {
+// commit != 0: the last block to finish also does O10 (t += 1), which saves the one-thread k_commit launch
+__global__ void __launch_bounds__(128) k_advance(const AxgParams p, int commit) {
     AxgDev* dev = p.dev;
     const uint32_t t = dev->step;
     const AxgRoundKeys rk = axg_round_keys(p.seed_lo, p.seed_hi);
@@ -132,6 +133,10 @@ __global__ void __launch_bounds__(128) k_advance(const AxgParams p) {
         }
         if (state) p.cone_state[c] = state;
     }
+    if (commit && axg_last_block(dev) && threadIdx.x == 0) {  // every block has read dev->step by now
+        dev->done = 0u;
+        dev->step = t + 1u;
+    }
 }
 
 __global__ void k_commit(const AxgParams p) { p.dev->step += 1u; }  // O10
@@ -194,9 +199,9 @@ void axg_launch_sense(const AxgParams& p, cudaStream_t s) {
     if (!p.n_cones) return;
     k_sense<<<grid_for(p.n_cones, 8, 148 * 8), 256, 0, s>>>(p);
 }
-void axg_launch_advance(const AxgParams& p, cudaStream_t s) {
+void axg_launch_advance(const AxgParams& p, int commit, cudaStream_t s) {
     if (!p.n_cones) return;
-    k_advance<<<grid_for(p.n_cones, 128, 148 * 16), 128, 0, s>>>(p);
+    k_advance<<<grid_for(p.n_cones, 128, 148 * 16), 128, 0, s>>>(p, commit);
 }
 void axg_launch_commit(const AxgParams& p, cudaStream_t s) { k_commit<<<1, 1, 0, s>>>(p); }
 void axg_launch_census(const AxgParams& p, cudaStream_t s) {

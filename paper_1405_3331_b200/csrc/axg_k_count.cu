@@ -192,7 +192,8 @@ __global__ void __launch_bounds__(SETTLE_THREADS, 6) k_settle(const AxgParams p)
             const uint32_t k = axg_cell_key(p, r[i].x, r[i].y, r[i].z);
             const uint32_t lo = __ldg(cell_lo + k), hi = __ldg(cell_lo + k + 1u);
             uint32_t rank = 0u;  // members of my cell with a smaller pre-sort index (reading A-9: ties keep that order)
-            for (uint32_t q = lo; q < hi; ++q) rank += ((__ldg(slot + q) & AXG_IDX_MASK) < idx) ? 1u : 0u;
+            if (hi - lo > 1u)  // alone in the cell (the common case): nothing to rank against
+                for (uint32_t q = lo; q < hi; ++q) rank += ((__ldg(slot + q) & AXG_IDX_MASK) < idx) ? 1u : 0u;
             const uint32_t dst = lo + rank;
             p.A.x[dst] = r[i].x;
             p.A.y[dst] = r[i].y;
