@@ -41,7 +41,9 @@ HBM_FALLBACK_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md "FALLBACK"
 NOMINAL_GBS = 8000.0          # north_star's "~8 TB/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the `ncu --set full` capture
 # summarised in profiles/ (a capture is not repeatable inside a timed run, so it is a recorded number).
-TRAFFIC_NCU = {}
+TRAFFIC_NCU = {   # (workload, kernel) -> bytes per launch; profiles/r01_summary.md
+    ("C3", "k_diffuse"): 703.0e6, ("C3", "k_settle"): 791.8e6, ("C3", "k_place"): 341.0e6, ("C3", "k_cell_scan"): 142.1e6,
+}
 
 
 def log(*a):
