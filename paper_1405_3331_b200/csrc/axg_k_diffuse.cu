@@ -174,25 +174,7 @@ __global__ void __launch_bounds__(DIFF_THREADS, 3) k_diffuse(const AxgParams p) 
                 if (lane == 0) axg_st_state(p.tile_state + tile, axg_pack(epoch, AXG_FLAG_INCL, ttotal));
             } else {
                 if (lane == 0) axg_st_state(p.tile_state + tile, axg_pack(epoch, AXG_FLAG_AGG, ttotal));
-                int q = (int)tile - 1 - lane;
-                while (true) {
-                    unsigned long long w;
-                    uint32_t f;
-                    do {
-                        w = (q >= 0) ? axg_ld_state(p.tile_state + q) : axg_pack(epoch, AXG_FLAG_INCL, 0u);
-                        f = axg_flag(w, epoch);
-                    } while (__any_sync(0xffffffffu, f == 0u));
-                    const uint32_t incl = __ballot_sync(0xffffffffu, f == (uint32_t)AXG_FLAG_INCL);
-                    uint32_t v = (uint32_t)w;
-                    if (incl) {
-                        const int firstincl = __ffs(incl) - 1;
-                        v = (lane <= firstincl) ? v : 0u;
-                        excl += __reduce_add_sync(0xffffffffu, v);
-                        break;
-                    }
-                    excl += __reduce_add_sync(0xffffffffu, v);
-                    q -= 32;
-                }
+                excl = axg_lookback(p.tile_state, tile, epoch, lane);
                 if (lane == 0) axg_st_state(p.tile_state + tile, axg_pack(epoch, AXG_FLAG_INCL, excl + ttotal));
             }
             if (lane == 0) {
