@@ -102,8 +102,11 @@ __device__ void emit_and_close(const AxgParams& p, int do_emit, uint32_t (*s_his
 
 __global__ void __launch_bounds__(DIFF_THREADS, 3) k_diffuse(const AxgParams p) {
     __shared__ uint32_t s_hist[AXG_MAX_PASSES][AXG_RADIX];
+    __shared__ float4 s_rec[DIFF_TILE];     // the tile's survivors, compacted inside the tile, waiting for their base
+    __shared__ uint32_t s_key[DIFF_TILE];
+    __shared__ uint8_t s_sp[DIFF_TILE];
     __shared__ uint32_t s_warp[DIFF_WARPS];
-    __shared__ uint32_t s_tile, s_base;
+    __shared__ uint32_t s_tk[2], s_base;
 
     AxgDev* dev = p.dev;
     const uint32_t n_in = dev->n_live, t = dev->step, epoch = dev->epoch;
@@ -113,79 +116,98 @@ __global__ void __launch_bounds__(DIFF_THREADS, 3) k_diffuse(const AxgParams p) 
     const AxgRoundKeys rk = axg_round_keys(p.seed_lo, p.seed_hi);
 
     for (int i = tid; i < AXG_MAX_PASSES * AXG_RADIX; i += DIFF_THREADS) (&s_hist[0][0])[i] = 0u;
+    if (tid == 0) s_tk[0] = atomicAdd(&dev->ticket, 1u);
+    __syncthreads();
 
+    // The chained compaction is software-pipelined over the tiles of a block: tile T's survivors are parked in shared
+    // memory and its aggregate is published at once, but its look-back -- which has to wait for EVERY tile in flight
+    // before it -- is resolved only after the arithmetic of the block's next tile, when those predecessors have long
+    // published.  (Resolving it right away cost ~40 polls per tile with all eight warps parked at a barrier.)
+    bool pending = false;
+    uint32_t ptile = 0u, ptotal = 0u;
+    int par = 0;
     while (true) {
-        __syncthreads();  // s_tile / s_warp / s_base reuse, and s_hist zeroing on the first trip
-        if (tid == 0) s_tile = atomicAdd(&dev->ticket, 1u);
-        __syncthreads();
-        const uint32_t tile = s_tile;
-        if (tile >= n_tiles) break;
+        const uint32_t tile = s_tk[par];
+        const bool have = tile < n_tiles;
+        if (tid == 0) s_tk[par ^ 1] = atomicAdd(&dev->ticket, 1u);  // next trip's tile, drawn a trip ahead
 
-        // ---- load: warp-striped, 128 B per warp request per column -------------------------------------
-        const uint32_t first = tile * DIFF_TILE + warp * (32 * DIFF_ITEMS) + lane;
         float x[DIFF_ITEMS], y[DIFF_ITEMS], z[DIFF_ITEMS];
         uint32_t id[DIFF_ITEMS];
         uint32_t sp_pack[DIFF_ITEMS / 4];
+        uint32_t alive = 0u, wtotal = 0u;
+        if (have) {
+            // ---- load: warp-striped, 128 B per warp request per column ---------------------------------------
+            const uint32_t first = tile * DIFF_TILE + warp * (32 * DIFF_ITEMS) + lane;
 #pragma unroll
-        for (int k = 0; k < DIFF_ITEMS / 4; ++k) sp_pack[k] = 0u;
+            for (int k = 0; k < DIFF_ITEMS / 4; ++k) sp_pack[k] = 0u;
 #pragma unroll
-        for (int i = 0; i < DIFF_ITEMS; ++i) {
-            const uint32_t g = first + i * 32;
-            const bool v = g < n_in;
-            x[i] = v ? __ldg(p.A.x + g) : -1.0f;
-            y[i] = v ? __ldg(p.A.y + g) : -1.0f;
-            z[i] = v ? __ldg(p.A.z + g) : -1.0f;
-            id[i] = v ? __ldg(p.A.id + g) : 0u;
-            const uint32_t s = v ? (uint32_t)__ldg(p.A.species + g) : 0u;
-            sp_pack[i >> 2] |= s << (8 * (i & 3));
+            for (int i = 0; i < DIFF_ITEMS; ++i) {
+                const uint32_t g = first + i * 32;
+                const bool v = g < n_in;
+                x[i] = v ? __ldg(p.A.x + g) : -1.0f;
+                y[i] = v ? __ldg(p.A.y + g) : -1.0f;
+                z[i] = v ? __ldg(p.A.z + g) : -1.0f;
+                id[i] = v ? __ldg(p.A.id + g) : 0u;
+                const uint32_t s = v ? (uint32_t)__ldg(p.A.species + g) : 0u;
+                sp_pack[i >> 2] |= s << (8 * (i & 3));
+            }
+            // ---- O1: diffuse; P1b: absorb -----------------------------------------------------------------------
+#pragma unroll
+            for (int i = 0; i < DIFF_ITEMS; ++i) {
+                const bool v = (first + i * 32) < n_in;
+                float z0, z1, z2;
+                axg_normals3(id[i], t, 0u, rk, z0, z1, z2);
+                x[i] = fmaf(p.sigma, z0, x[i]);
+                y[i] = fmaf(p.sigma, z1, y[i]);
+                z[i] = fmaf(p.sigma, z2, z[i]);
+                const bool in = x[i] >= 0.0f && x[i] < p.fnx && y[i] >= 0.0f && y[i] < p.fny && z[i] >= 0.0f &&
+                                z[i] < p.fnz;
+                alive |= (v && in) ? (1u << i) : 0u;
+            }
+            // ---- P1d: order-preserving ranks.  Order inside a warp chunk is (item, lane) = memory order. -----------
+#pragma unroll
+            for (int i = 0; i < DIFF_ITEMS; ++i) wtotal += __popc(__ballot_sync(0xffffffffu, (alive >> i) & 1u));
+            if (lane == 0) s_warp[warp] = wtotal;
         }
-
-        // ---- O1: diffuse; P1b: absorb ---------------------------------------------------------------------
-        uint32_t alive = 0u;
-#pragma unroll
-        for (int i = 0; i < DIFF_ITEMS; ++i) {
-            const bool v = (first + i * 32) < n_in;
-            float z0, z1, z2;
-            axg_normals3(id[i], t, 0u, rk, z0, z1, z2);
-            x[i] = fmaf(p.sigma, z0, x[i]);
-            y[i] = fmaf(p.sigma, z1, y[i]);
-            z[i] = fmaf(p.sigma, z2, z[i]);
-            const bool in = x[i] >= 0.0f && x[i] < p.fnx && y[i] >= 0.0f && y[i] < p.fny && z[i] >= 0.0f &&
-                            z[i] < p.fnz;
-            alive |= (v && in) ? (1u << i) : 0u;
-        }
-
-        // ---- P1d: order-preserving ranks.  Order inside a warp chunk is (item, lane) = memory order. ---------
-        uint32_t wtotal = 0u;
-#pragma unroll
-        for (int i = 0; i < DIFF_ITEMS; ++i) wtotal += __popc(__ballot_sync(0xffffffffu, (alive >> i) & 1u));
-        if (lane == 0) s_warp[warp] = wtotal;
-        __syncthreads();
+        __syncthreads();  // barrier A: warp totals
         uint32_t woff = 0u, ttotal = 0u;
+        if (have) {
 #pragma unroll
-        for (int w = 0; w < DIFF_WARPS; ++w) {
-            const uint32_t c = s_warp[w];
-            woff += (w < warp) ? c : 0u;
-            ttotal += c;
-        }
-        if (warp == 0) {  // decoupled look-back, 32 predecessors per probe
-            uint32_t excl = 0u;
-            if (tile == 0) {
-                if (lane == 0) axg_st_state(p.tile_state + tile, axg_pack(epoch, AXG_FLAG_INCL, ttotal));
-            } else {
-                if (lane == 0) axg_st_state(p.tile_state + tile, axg_pack(epoch, AXG_FLAG_AGG, ttotal));
-                excl = axg_lookback(p.tile_state, tile, epoch, lane);
-                if (lane == 0) axg_st_state(p.tile_state + tile, axg_pack(epoch, AXG_FLAG_INCL, excl + ttotal));
+            for (int w = 0; w < DIFF_WARPS; ++w) {
+                const uint32_t c = s_warp[w];
+                woff += (w < warp) ? c : 0u;
+                ttotal += c;
             }
-            if (lane == 0) {
-                s_base = excl;
-                if (tile == n_tiles - 1) dev->n_surv = excl + ttotal;
-            }
+            if (tid == 0)  // tile 0 has nothing before it: its aggregate is its inclusive prefix
+                axg_st_state(p.tile_state + tile, axg_pack(epoch, tile == 0 ? AXG_FLAG_INCL : AXG_FLAG_AGG, ttotal));
         }
-        __syncthreads();
-        uint32_t out = s_base + woff;
-
-        // ---- write survivors (coalesced: consecutive lanes -> consecutive slots), key, histograms -------------
+        // ---- the parked tile: look-back (its predecessors had a whole tile's time to publish), then flush ----------
+        if (pending) {
+            if (warp == 0) {
+                uint32_t excl = 0u;
+                if (ptile > 0) {
+                    excl = axg_lookback(p.tile_state, ptile, epoch, lane);
+                    if (lane == 0) axg_st_state(p.tile_state + ptile, axg_pack(epoch, AXG_FLAG_INCL, excl + ptotal));
+                }
+                if (lane == 0) {
+                    s_base = excl;
+                    if (ptile == n_tiles - 1) dev->n_surv = excl + ptotal;
+                }
+            }
+            __syncthreads();  // barrier B: base known
+            const uint32_t base = s_base;
+            for (uint32_t q = tid; q < ptotal; q += DIFF_THREADS) {  // contiguous in global memory: 128-bit records
+                p.Brec[base + q] = s_rec[q];
+                p.key_pre[base + q] = s_key[q];
+                p.Bsp[base + q] = s_sp[q];
+            }
+            __syncthreads();  // barrier C: the parking area is free
+        } else {
+            __syncthreads();  // first trip: s_warp has been read by everyone before the next trip rewrites it
+        }
+        if (!have) break;
+        // ---- park my survivors at their tile-local slots; key; histograms / cell counts ---------------------------
+        uint32_t out = woff;
 #pragma unroll
         for (int i = 0; i < DIFF_ITEMS; ++i) {
             const uint32_t a = (alive >> i) & 1u;
@@ -193,13 +215,17 @@ __global__ void __launch_bounds__(DIFF_THREADS, 3) k_diffuse(const AxgParams p) 
             if (a) {
                 const uint32_t o = out + __popc(b & lt);
                 const uint32_t key = axg_cell_key(p, x[i], y[i], z[i]);
-                p.Brec[o] = make_float4(x[i], y[i], z[i], __uint_as_float(id[i]));
-                p.Bsp[o] = (uint8_t)((sp_pack[i >> 2] >> (8 * (i & 3))) & 0xffu);
-                p.key_pre[o] = key;
+                s_rec[o] = make_float4(x[i], y[i], z[i], __uint_as_float(id[i]));
+                s_sp[o] = (uint8_t)((sp_pack[i >> 2] >> (8 * (i & 3))) & 0xffu);
+                s_key[o] = key;
                 tally(p, s_hist, key);
             }
             out += __popc(b);
         }
+        pending = true;
+        ptile = tile;
+        ptotal = ttotal;
+        par ^= 1;
     }
 
     __syncthreads();
