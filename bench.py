@@ -236,7 +236,8 @@ def run_ours(args, w):
     seed = w.seed
 
     bin_req = {"auto": axg.BIN_AUTO, "radix": axg.BIN_RADIX, "count": axg.BIN_COUNT}[args.binning]
-    count_mode = bin_req == axg.BIN_COUNT or (bin_req == axg.BIN_AUTO and w.cells <= 4 * (w.max_particles or 1 << 20))
+    count_mode = bin_req == axg.BIN_COUNT or (bin_req == axg.BIN_AUTO and w.cells <= axg.AUTO_COUNT_MAX_CELLS and
+                                              w.cells <= 4 * (w.max_particles or 1 << 20))
 
     def make_sim(D, emission):
         sim_ = axg.Axg(w.grid, D, emission, w.radius, w.speed, w.noise, seed)

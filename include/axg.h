@@ -170,9 +170,11 @@ int axg_set_shard(axg_ctx* ctx, uint32_t rank, uint32_t world);
  *  AXG_BIN_COUNT  counting sort over the cells: P1 counts particles per cell (one L2 atomic each), a single-pass
  *                 scan over the cells gives the cell ranges, and a rank-inside-the-cell kernel restores the stable
  *                 order.  Cost ~ N + cells; 4 B x cells of extra device memory.
- *  AXG_BIN_AUTO   (default) COUNT when cells <= 4 x particle capacity, else RADIX.
+ *  AXG_BIN_AUTO   (default) COUNT when cells <= AXG_AUTO_COUNT_MAX_CELLS (the count array fits the L2 cache) and
+ *                 cells <= 4 x particle capacity, else RADIX.
  * Allowed whenever no step is half done (not between AXG_PHASE_DIFFUSE and AXG_PHASE_BIN): AXG_ESTATE.    */
 enum { AXG_BIN_AUTO = 0, AXG_BIN_RADIX = 1, AXG_BIN_COUNT = 2 };
+#define AXG_AUTO_COUNT_MAX_CELLS 20000000u
 int axg_set_binning(axg_ctx* ctx, int mode);
 
 /* Device pointer (int32[C][AXG_MAX_SPECIES][4] = n,Mx,My,Mz) of the per-cone sensing sums, for the NCCL

@@ -222,7 +222,11 @@ int alloc_particles(axg_ctx* c, uint64_t cap, AxgParams& P, std::vector<void*>& 
 // AXG_BIN_AUTO -> a concrete mode; the count array exists (all-zero) whenever the mode is COUNT
 int resolve_binning(axg_ctx* c) {
     int mode = c->bin_request;
-    if (mode == AXG_BIN_AUTO) mode = (c->cells() <= 4 * (size_t)c->max_particles) ? AXG_BIN_COUNT : AXG_BIN_RADIX;
+    // count mode pays per cell and wants its 4 B x cells count array resident in the 126 MB L2 (measured: faster than
+    // radix at C3 = 16.8 M cells, slower at C4 = 134 M cells, where its atomics go to DRAM)
+    if (mode == AXG_BIN_AUTO)
+        mode = (c->cells() <= AXG_AUTO_COUNT_MAX_CELLS && c->cells() <= 4 * (size_t)c->max_particles) ? AXG_BIN_COUNT
+                                                                                                      : AXG_BIN_RADIX;
     if (mode == AXG_BIN_COUNT && !c->d_cnt) {
         c->d_cnt = dev_alloc(c, c->cells_padded() * sizeof(uint32_t));
         c->d_scan_state = dev_alloc(c, c->scan_tiles() * sizeof(unsigned long long));

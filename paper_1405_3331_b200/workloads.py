@@ -84,7 +84,7 @@ def c3(rate=350):
                     timed_steps=500, prerun_steps=22000, max_particles=24_000_000, max_segments=1200)
 
 
-def c4(rate=140):
+def c4(rate=100):
     """512^3, 100k cones in 32 Gaussian clusters on z<8, 64 sources in 8 Gaussian blobs, two species, D=1, R=3."""
     rng = np.random.default_rng(1004)
     centres = np.stack([rng.uniform(16, 496, 32), rng.uniform(16, 496, 32), rng.uniform(0, 8, 32)], 1)
@@ -102,7 +102,7 @@ def c4(rate=140):
         sp = i % 2
         sources.append((float(q[0]), float(q[1]), float(q[2]), sp, 1 if sp == 0 else -1, rate))
     return Workload("C4", (512, 512, 512), 1.0, rate, 3.0, 0.5, 0.05, 4, neurons, sources, nominal_live=64_000_000,
-                    timed_steps=200, prerun_steps=45000, max_particles=80_000_000, max_segments=400)
+                    timed_steps=200, prerun_steps=45000, max_particles=120_000_000, max_segments=400)
 
 
 def c5(rate=110):
@@ -227,7 +227,9 @@ def prerun(make_sim, w: Workload, coarse=16, relax=100, progress=None):
         while todo > 0:
             # the boundary refuses a call whose host-side bound n_live + k * E could overflow the capacity
             n_live = pre.counters()["n_live"]
-            k = int(min(todo, 256, max(1, (cap - n_live) // max(e_coarse, 1))))
+            k = int(min(todo, 256, (cap - n_live) // max(e_coarse, 1)))
+            if k < 1:       # the capacity is reached before the steady state: hand over what there is
+                break
             pre.step(k)
             todo -= k
             if progress:
