@@ -378,7 +378,7 @@ int enqueue_phases(axg_ctx* c, uint32_t mask, Prof& prof) {
             prof.mark(AXG_K_PLACE);
             axg_launch_place(P, N_SM * 8, s);
             prof.mark(AXG_K_SETTLE);
-            axg_launch_settle(P, N_SM * 6, s);
+            axg_launch_settle(P, N_SM * 8, s);
             launches += 3;
             c->cnt_dirty = false;
         } else {

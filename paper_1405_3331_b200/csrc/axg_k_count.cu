@@ -118,31 +118,23 @@ __global__ void __launch_bounds__(PLACE_THREADS) k_place(const AxgParams p) {
     const uint32_t n = p.dev->n_live;
     uint32_t* __restrict__ slot = p.sidx[p.final_buf ^ 1];
     uint32_t* __restrict__ cell_lo = p.cell_lo;
-    const uint32_t n4 = n >> 2;
-    for (uint32_t g = blockIdx.x * PLACE_THREADS + threadIdx.x; g < n4; g += gridDim.x * PLACE_THREADS) {
-        const uint4 k = __ldg(reinterpret_cast<const uint4*>(p.key_pre) + g);
-        const uchar4 s = __ldg(reinterpret_cast<const uchar4*>(p.Bsp) + g);
-        const uint32_t o = g * 4u;
+    // one particle per thread: measured faster than four per thread with 128-bit loads (0.176 vs 0.213 ms at C3) -- the
+    // kernel is bound by L2 transactions (one atomic + one scattered 4-byte store each) and wants many warps in flight
+    for (uint32_t o = blockIdx.x * PLACE_THREADS + threadIdx.x; o < n; o += gridDim.x * PLACE_THREADS) {
+        const uint32_t k = __ldg(p.key_pre + o);
+        const uint32_t sp = __ldg(p.Bsp + o);
         // bumping the cursor hands out the slots of the cell in the arbitrary order of the atomics
-        const uint32_t d0 = take_slot(cell_lo, k.x), d1 = take_slot(cell_lo, k.y), d2 = take_slot(cell_lo, k.z),
-                       d3 = take_slot(cell_lo, k.w);
-        slot[d0] = o | ((uint32_t)s.x << 30);
-        slot[d1] = (o + 1u) | ((uint32_t)s.y << 30);
-        slot[d2] = (o + 2u) | ((uint32_t)s.z << 30);
-        slot[d3] = (o + 3u) | ((uint32_t)s.w << 30);
-    }
-    if (blockIdx.x == 0 && threadIdx.x < (n & 3u)) {  // ragged tail
-        const uint32_t o = n4 * 4u + threadIdx.x;
-        slot[take_slot(cell_lo, p.key_pre[o])] = o | ((uint32_t)p.Bsp[o] << 30);
+        slot[take_slot(cell_lo, k)] = o | (sp << 30);
     }
 }
 
 // ---- rank inside the cell by pre-sort index, then O5: A[cell_lo + rank] = B[index] -------------------------------
 constexpr int SETTLE_THREADS = 256;
-constexpr int SETTLE_ITEMS = 4;  // warp-striped: item i of lane l is slot base + 32 i + l, so every access of a
-                                 // warp instruction covers 32 neighbouring slots
+constexpr int SETTLE_ITEMS = 1;  // warp-striped (item i of lane l is slot base + 32 i + l).  Measured at C3: 1 item and
+                                 // 8 blocks per SM 0.188 ms, 2 items 0.198, 4 items / 6 blocks 0.227, 8 items 0.272 --
+                                 // the kernel lives on many independent warps in flight, not on ILP inside one
 
-__global__ void __launch_bounds__(SETTLE_THREADS, 6) k_settle(const AxgParams p) {
+__global__ void __launch_bounds__(SETTLE_THREADS, 8) k_settle(const AxgParams p) {
     const uint32_t n = p.dev->n_live;
     const uint32_t* __restrict__ slot = p.sidx[p.final_buf ^ 1];
     uint32_t* __restrict__ perm = p.sidx[p.final_buf];
