@@ -28,6 +28,8 @@ struct Source {
 };
 
 constexpr int N_SM = 148;
+// k_reorder variant: four slots per thread when the particle streams cannot live in the L2 (see axg_k_bin.cu)
+constexpr uint64_t AXG_REORDER_WIDE_ABOVE = 32ull << 20;
 
 }  // namespace
 
@@ -360,7 +362,7 @@ int enqueue_phases(axg_ctx* c, uint32_t mask, Prof& prof) {
     if (mask & AXG_PHASE_DIFFUSE) {
         zero_cnt_if_dirty();
         prof.mark(AXG_K_DIFFUSE);
-        axg_launch_diffuse(P, N_SM * 3, s);  // its last block emits and closes P1
+        axg_launch_diffuse(P, N_SM * 4, s);  // its last block emits and closes P1
         launches += 1;
         c->cnt_dirty = count_mode;
     }
@@ -385,7 +387,7 @@ int enqueue_phases(axg_ctx* c, uint32_t mask, Prof& prof) {
             prof.mark(AXG_K_SORT);
             for (int q = 0; q < P.n_pass; ++q) axg_launch_sort_pass(P, q, N_SM * 2, s);
             prof.mark(AXG_K_REORDER);
-            axg_launch_reorder(P, N_SM * 8, s);
+            axg_launch_reorder(P, N_SM * 8, c->max_particles > AXG_REORDER_WIDE_ABOVE ? 1 : 0, s);
             launches += P.n_pass + 1;
         }
     }

@@ -108,6 +108,21 @@ def test_binning_only_on_given_positions(axg):
         o.close()
 
 
+def test_binning_with_the_wide_reorder_kernel(axg):
+    """A particle capacity above 32 M selects the four-slots-per-thread reorder kernel (radix mode): same results."""
+    grid, n, seed = (64, 48, 40), 123_457, 5
+    g = pu.new_axg(axg, grid, 0.5, 1, 2.0, 0.25, 0.1, seed)
+    o = axo.Oracle(grid, 0.5, 1, 2.0, 0.25, 0.1, seed)
+    g.set_capacity(34_000_000, 8)
+    o.set_capacity(34_000_000, 8)
+    load_same_particles(g, o, seed, n, grid)
+    g.step_phase(axg.PHASE_BIN)
+    o.step_phase(axo.PHASE_BIN)
+    compare_binning(g, o)
+    g.close()
+    o.close()
+
+
 def test_table1_of_the_paper_on_gpu(axg, golden_dir):
     """PAPER.md:267-276 Table 1 (reading A-17): 6 particles in cells 9 6 6 4 6 4 of a 16-cell row."""
     cells = np.array([9, 6, 6, 4, 6, 4])
