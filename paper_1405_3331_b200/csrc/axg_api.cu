@@ -46,6 +46,10 @@ struct axg_ctx {
     uint32_t n_cones = 0;
     bool stepped = false;
     cudaStream_t stream = nullptr;
+    // P3..P5 of step t run on a side stream while k_diffuse of step t+1 runs on `stream` (axg_step only)
+    cudaStream_t side = nullptr;
+    cudaEvent_t ev_bin = nullptr, ev_adv = nullptr;
+    bool adv_pending = false;
     std::string err;
 
     // device memory
@@ -351,7 +355,7 @@ struct Prof {
 };
 
 // enqueue the selected phases of one step; returns the number of kernel launches
-int enqueue_phases(axg_ctx* c, uint32_t mask, Prof& prof) {
+int enqueue_phases(axg_ctx* c, uint32_t mask, Prof& prof, bool overlap = false) {
     const AxgParams& P = c->P;
     cudaStream_t s = c->stream;
     int launches = 0;
@@ -367,6 +371,8 @@ int enqueue_phases(axg_ctx* c, uint32_t mask, Prof& prof) {
         c->cnt_dirty = count_mode;
     }
     if (mask & AXG_PHASE_BIN) {
+        // the previous step's P3 (side stream) still reads cell_lo and the species column that P2 rewrites
+        if (overlap && c->adv_pending) cudaStreamWaitEvent(s, c->ev_adv, 0);
         if (!(mask & AXG_PHASE_DIFFUSE)) {
             zero_cnt_if_dirty();
             prof.mark(AXG_K_EMIT);
@@ -391,21 +397,34 @@ int enqueue_phases(axg_ctx* c, uint32_t mask, Prof& prof) {
             launches += P.n_pass + 1;
         }
     }
+    cudaStream_t sc = s;  // stream of the cone kernels
+    if (overlap) {
+        cudaEventRecord(c->ev_bin, s);
+        cudaStreamWaitEvent(c->side, c->ev_bin, 0);
+        sc = c->side;
+    }
     if ((mask & AXG_PHASE_SENSE) && P.n_cones) {
         prof.mark(AXG_K_SENSE);
-        axg_launch_sense(P, s);
+        axg_launch_sense(P, sc);
         launches += 1;
     }
     bool committed = false;
     if ((mask & AXG_PHASE_ADVANCE) && P.n_cones) {
         prof.mark(AXG_K_ADVANCE);
         committed = (mask & AXG_PHASE_COMMIT) != 0;  // O10 rides in the last block of k_advance
-        axg_launch_advance(P, committed ? 1 : 0, s);
+        axg_launch_advance(P, committed ? 1 : 0, sc);
         launches += 1;
+    }
+    if (overlap) {
+        cudaEventRecord(c->ev_adv, c->side);
+        c->adv_pending = true;
     }
     if ((mask & AXG_PHASE_COMMIT) && !committed) {
         prof.mark(AXG_K_COMMIT);
-        axg_launch_commit(P, s);
+        axg_launch_commit(P, 1, s);
+        launches += 1;
+    } else if (committed && !(mask & AXG_PHASE_DIFFUSE)) {  // phase calls: keep P1's step index aligned
+        axg_launch_commit(P, 0, sc);
         launches += 1;
     }
     return launches;
@@ -486,6 +505,9 @@ AXG_API void axg_destroy(axg_ctx* c) {
     dev_free(c->d_dev); dev_free(c->d_cell_lo); dev_free(c->d_src); dev_free(c->d_src_id_prefix);
     dev_free(c->d_src_emit_prefix); dev_free(c->d_stencil);
     for (cudaEvent_t e : c->prof_events) cudaEventDestroy(e);
+    if (c->ev_bin) cudaEventDestroy(c->ev_bin);
+    if (c->ev_adv) cudaEventDestroy(c->ev_adv);
+    if (c->side) cudaStreamDestroy(c->side);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
     delete c;
@@ -628,6 +650,7 @@ AXG_API int axg_load_particles(axg_ctx* c, const float* x, const float* y, const
     CU(c, cudaMemcpyAsync(&d->n_live, &n32, 4, cudaMemcpyHostToDevice, c->stream));
     CU(c, cudaMemcpyAsync(&d->next_id, &next_id, 4, cudaMemcpyHostToDevice, c->stream));
     CU(c, cudaMemcpyAsync(&d->step, &step, 4, cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaMemcpyAsync(&d->pstep, &step, 4, cudaMemcpyHostToDevice, c->stream));
     CU(c, cudaStreamSynchronize(c->stream));
     c->n_A = n32;
     c->loaded_species_mask = mask;
@@ -664,8 +687,20 @@ AXG_API int axg_step(axg_ctx* c, uint32_t n) {
     Prof prof{c, c->profile_next};
     c->profile_next = false;
     uint64_t launches = 0;
+    // With cones and no per-kernel profiling, P3..P5 of step t overlap k_diffuse of step t+1 (they share nothing:
+    // P1 draws its step index from AxgDev::pstep, P3..P5 commit AxgDev::step).
+    const bool overlap = c->n_cones > 0 && !prof.on && n > 1;
+    if (overlap && !c->side) {
+        CU(c, cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking));
+        CU(c, cudaEventCreateWithFlags(&c->ev_bin, cudaEventDisableTiming));
+        CU(c, cudaEventCreateWithFlags(&c->ev_adv, cudaEventDisableTiming));
+    }
     CU(c, cudaEventRecord(c->ev0, c->stream));
-    for (uint32_t i = 0; i < n; ++i) launches += enqueue_phases(c, AXG_PHASE_ALL, prof);
+    for (uint32_t i = 0; i < n; ++i) launches += enqueue_phases(c, AXG_PHASE_ALL, prof, overlap);
+    if (c->adv_pending) {  // join: the ctx stream waits for the last step's cones
+        CU(c, cudaStreamWaitEvent(c->stream, c->ev_adv, 0));
+        c->adv_pending = false;
+    }
     prof.mark(-1);
     CU(c, cudaEventRecord(c->ev1, c->stream));
     c->stepped = true;

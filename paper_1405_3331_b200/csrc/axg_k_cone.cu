@@ -133,13 +133,17 @@ __global__ void __launch_bounds__(128) k_advance(const AxgParams p, int commit) 
         }
         if (state) p.cone_state[c] = state;
     }
-    if (commit && axg_last_block(dev) && threadIdx.x == 0) {  // every block has read dev->step by now
-        dev->done = 0u;
-        dev->step = t + 1u;
+    if (commit && axg_last_block(&dev->done2) && threadIdx.x == 0) {  // every block has read dev->step by now
+        dev->done2 = 0u;
+        dev->step = t + 1u;  // NOT pstep: the next step's P1 may already have bumped it (see AxgDev::pstep)
     }
 }
 
-__global__ void k_commit(const AxgParams p) { p.dev->step += 1u; }  // O10
+// O10; bump == 0: only re-align P1's step index with the committed one (phase calls that commit without a P1)
+__global__ void k_commit(const AxgParams p, int bump) {
+    p.dev->step += (uint32_t)bump;
+    p.dev->pstep = p.dev->step;
+}
 
 __global__ void k_census(const AxgParams p) {
     __shared__ uint32_t s_c[4];
@@ -203,7 +207,7 @@ void axg_launch_advance(const AxgParams& p, int commit, cudaStream_t s) {
     if (!p.n_cones) return;
     k_advance<<<grid_for(p.n_cones, 128, 148 * 16), 128, 0, s>>>(p, commit);
 }
-void axg_launch_commit(const AxgParams& p, cudaStream_t s) { k_commit<<<1, 1, 0, s>>>(p); }
+void axg_launch_commit(const AxgParams& p, int bump, cudaStream_t s) { k_commit<<<1, 1, 0, s>>>(p, bump); }
 void axg_launch_census(const AxgParams& p, cudaStream_t s) {
     if (!p.n_cones) return;
     k_census<<<grid_for(p.n_cones, 256, 148 * 4), 256, 0, s>>>(p);

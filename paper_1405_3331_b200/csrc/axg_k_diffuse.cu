@@ -92,7 +92,8 @@ __device__ void emit_and_close(const AxgParams& p, int do_emit, uint32_t (*s_his
         }
     }
     if (tid == 0 && do_emit) {
-        if (!fits) dev->err |= 1u;
+        dev->pstep += 1u;  // P1 of step t is done: the next k_diffuse draws from (id, t + 1)
+        if (!fits) atomicOr(&dev->err, 1u);
         dev->n_live = fits ? n_surv + p.e_owned : n_surv;
         dev->next_id = next_id + p.e_total;
         dev->emitted += fits ? p.e_owned : 0u;
@@ -110,7 +111,7 @@ __global__ void __launch_bounds__(DIFF_THREADS, 4) k_diffuse(const AxgParams p) 
     __shared__ uint32_t s_tk[2], s_base;
 
     AxgDev* dev = p.dev;
-    const uint32_t n_in = dev->n_live, t = dev->step, epoch = dev->epoch;
+    const uint32_t n_in = dev->n_live, t = dev->pstep, epoch = dev->epoch;
     const uint32_t n_tiles = (n_in + DIFF_TILE - 1) / DIFF_TILE;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t lt = axg_lanemask_lt();
