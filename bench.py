@@ -69,7 +69,7 @@ def key_passes(cells):
     return (bits + 7) // 8
 
 
-def bytes_model(w, n_live, n_active_cones, n_stencil, count_mode, fused_steps=0):
+def bytes_model(w, n_live, n_active_cones, n_stencil, count_mode):
     """Algorithmic bytes of ONE step at n_live particles.  `step` is SURVEY.md §8(d)'s figure for the
     METHOD (K1 38 + sort 12 + 16 (passes - 1) + reorder 42 per particle, 8 B per cell of cell-range upkeep, the cone
     bytes) and does not depend on how P2 is computed; the per-kernel entries are what each kernel of the chosen
@@ -86,14 +86,6 @@ def bytes_model(w, n_live, n_active_cones, n_stencil, count_mode, fused_steps=0)
              "settle": 53.0 * n_live,              # slot 4 + record 16 + cell_lo 8 + SoA 17 + key 4 + perm 4
              "sense": sense}
         launches = {"diffuse": 1, "scan": 1, "place": 1, "settle": 1, "sense": 1}
-        if fused_steps > 1:
-            # one axg_step(K) call = k_diffuse, (K - 1) x k_diffuse<fused>, k_settle: entries are per STEP, so the
-            # per-launch figure (entry / launches per step) stays 42 / 53 / 95 B per particle
-            f = (fused_steps - 1.0) / fused_steps
-            k["settle_diffuse"] = (53.0 + 42.0) * n_live * f   # what k_settle + k_diffuse must move between them
-            k["diffuse"] *= 1.0 - f
-            k["settle"] *= 1.0 - f
-            launches.update({"settle_diffuse": f, "diffuse": 1.0 - f, "settle": 1.0 - f})
     else:
         k = {"diffuse": 38.0 * n_live,
              "sort": (12.0 + 16.0 * (passes - 1)) * n_live,   # pass 0: 4 read + 8 write; later passes 8 + 8
@@ -247,12 +239,10 @@ def run_ours(args, w):
     bin_req = {"auto": axg.BIN_AUTO, "radix": axg.BIN_RADIX, "count": axg.BIN_COUNT}[args.binning]
     count_mode = bin_req == axg.BIN_COUNT or (bin_req == axg.BIN_AUTO and w.cells <= axg.AUTO_COUNT_MAX_CELLS and
                                               w.cells <= 4 * (w.max_particles or 1 << 20))
-    fused = count_mode and args.fusion != "off" and world == 1   # the sharded loop enqueues phase by phase
 
     def make_sim(D, emission):
         sim_ = axg.Axg(w.grid, D, emission, w.radius, w.speed, w.noise, seed)
         sim_.set_binning(bin_req)
-        sim_.set_fusion({"off": axg.FUSE_OFF, "on": axg.FUSE_ON, "materialize": axg.FUSE_MATERIALIZE}[args.fusion])
         if world > 1:
             sim_.set_shard(rank, world)   # every rank pre-runs its own shard: particle sets of sources never interact
         return sim_
@@ -325,11 +315,10 @@ def run_ours(args, w):
                     if dx * dx + dy * dy + dz * dz <= r2)
     extra = {}
     if ktimes is not None:
-        step_bytes, bm, launches_of = bytes_model(w, n_avg, active, n_stencil, count_mode, K if fused else 0)
+        step_bytes, bm, launches_of = bytes_model(w, n_avg, active, n_stencil, count_mode)
         per_step_ms = {k: v / K for k, v in ktimes.items()}
         kernel_name = {"diffuse": "k_diffuse", "sort": "k_sort_pass", "reorder": "k_reorder", "sense": "k_sense",
-                       "scan": "k_cell_scan", "place": "k_place", "settle": "k_settle",
-                       "settle_diffuse": "k_diffuse<fused>"}
+                       "scan": "k_cell_scan", "place": "k_place", "settle": "k_settle"}
         dom = max(bm.keys(), key=lambda k: per_step_ms[k])
         per_launch_ms = per_step_ms[dom] / launches_of[dom]
         per_launch_bytes = bm[dom] / launches_of[dom]
@@ -348,7 +337,6 @@ def run_ours(args, w):
         extra["kernels_gbs"] = {k: bm[k] / (per_step_ms[k] * 1e-3) / 1e9 for k in bm if per_step_ms[k] > 0}
         extra["cone_steps_per_s"] = active / (step_ms * 1e-3)
         extra["binning"] = "count" if count_mode else "radix"
-        extra["fusion"] = args.fusion if fused else "off"
 
     # ---- e2e: the same job through the C-ABI with HOST buffers; every host<->device copy inside the timed region --
     # upload of the particle SoA + cone state from pinned host memory, then e2e_steps x [axg_step(1), read back cone
@@ -444,8 +432,6 @@ def main():
     ap.add_argument("--coarse", type=int, default=16, help="coarse-time factor of the steady-state pre-run")
     ap.add_argument("--e2e-steps", type=int, default=20)
     ap.add_argument("--binning", default="auto", choices=("auto", "radix", "count"))
-    ap.add_argument("--fusion", default="on", choices=("off", "on", "materialize"),
-                    help="count binning: P2b/P2c of step t inside k_diffuse of step t+1 (include/axg.h axg_set_fusion)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     from paper_1405_3331_b200 import workloads as W

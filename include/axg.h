@@ -179,14 +179,6 @@ enum { AXG_BIN_AUTO = 0, AXG_BIN_RADIX = 1, AXG_BIN_COUNT = 2 };
 #define AXG_AUTO_COUNT_MAX_CELLS 20000000u
 int axg_set_binning(axg_ctx* ctx, int mode);
 
-/* Kernel fusion across steps inside axg_step(n > 1) with count binning: mode 1 (default) runs the
- * rank-inside-the-cell + reorder of step t (P2b/P2c) inside the diffusion kernel of step t+1, so the sorted SoA of an
- * inner step stays on chip; the SoA, sorted keys and permutation that axg_read_state reports are written by the
- * closing reorder kernel of the call.  Mode 2 = fused, and every inner step also stores them.  Mode 0 = one kernel
- * per phase.  Results are identical bit for bit in all modes.                                             */
-enum { AXG_FUSE_OFF = 0, AXG_FUSE_ON = 1, AXG_FUSE_MATERIALIZE = 2 };
-int axg_set_fusion(axg_ctx* ctx, int mode);
-
 /* Device pointer (int32[C][AXG_MAX_SPECIES][4] = n,Mx,My,Mz) of the per-cone sensing sums, for the NCCL
  * all-reduce between P3 and P4 when sharded.  *bytes = its size.  Owned by ctx.                           */
 int axg_sense_buffer(axg_ctx* ctx, void** device_ptr, size_t* bytes);
@@ -222,8 +214,7 @@ int axg_last_step_stats(axg_ctx* ctx, float* device_ms, uint64_t* launches, uint
  * hold AXG_KERNEL_COUNT floats after the call via axg_kernel_times.                                      */
 enum {
     AXG_K_CLEAR = 0, AXG_K_DIFFUSE = 1, AXG_K_EMIT = 2, AXG_K_SORT = 3, AXG_K_REORDER = 4, AXG_K_SENSE = 5,
-    AXG_K_ADVANCE = 6, AXG_K_COMMIT = 7, AXG_K_SCAN = 8, AXG_K_PLACE = 9, AXG_K_SETTLE = 10,
-    AXG_K_SETTLE_DIFFUSE = 11, AXG_KERNEL_COUNT = 12
+    AXG_K_ADVANCE = 6, AXG_K_COMMIT = 7, AXG_K_SCAN = 8, AXG_K_PLACE = 9, AXG_K_SETTLE = 10, AXG_KERNEL_COUNT = 11
 };
 int axg_profile_next_step(axg_ctx* ctx, int enable);
 int axg_kernel_times(axg_ctx* ctx, float* times_ms /* AXG_KERNEL_COUNT */);

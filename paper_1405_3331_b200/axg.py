@@ -26,17 +26,14 @@ _DTYPES = {
 }
 PHASE_DIFFUSE, PHASE_BIN, PHASE_SENSE, PHASE_ADVANCE, PHASE_COMMIT, PHASE_ALL = 1, 2, 4, 8, 16, 31
 COUNTER_NAMES = ("step", "n_live", "next_id", "emitted", "absorbed", "active", "arrived", "exited")
-KERNEL_NAMES = ("clear", "diffuse", "emit", "sort", "reorder", "sense", "advance", "commit", "scan", "place", "settle",
-                "settle_diffuse")
+KERNEL_NAMES = ("clear", "diffuse", "emit", "sort", "reorder", "sense", "advance", "commit", "scan", "place", "settle")
 BIN_AUTO, BIN_RADIX, BIN_COUNT = 0, 1, 2
-FUSE_OFF, FUSE_ON, FUSE_MATERIALIZE = 0, 1, 2
 AUTO_COUNT_MAX_CELLS = 20_000_000   # include/axg.h AXG_AUTO_COUNT_MAX_CELLS
 EXPORTS = (
     "axg_create", "axg_place_neurons", "axg_add_source", "axg_step", "axg_read_state", "axg_destroy",
     "axg_last_error", "axg_set_capacity", "axg_load_particles", "axg_load_cones", "axg_step_phase", "axg_set_shard",
     "axg_sense_buffer", "axg_set_stream", "axg_set_allocator", "axg_last_step_stats", "axg_profile_next_step",
     "axg_kernel_times", "axg_check_capacity", "axg_enqueue_phase", "axg_sync", "axg_set_binning",
-    "axg_set_fusion",
 )
 
 _ALLOC_T = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p)
@@ -87,7 +84,6 @@ def lib(build=True):
     L.axg_enqueue_phase.argtypes = [vp, u32]
     L.axg_sync.argtypes = [vp]
     L.axg_set_binning.argtypes = [vp, C.c_int]
-    L.axg_set_fusion.argtypes = [vp, C.c_int]
     L.axg_load_particles.argtypes = [vp, vp, vp, vp, vp, vp, u64, u32, u32]
     L.axg_load_cones.argtypes = [vp, vp, vp, vp, vp, u32]
     L.axg_read_state.argtypes = [vp, u32, vp, sz, C.POINTER(sz)]
@@ -186,9 +182,6 @@ class Axg:
 
     def set_binning(self, mode):
         self._chk(self._L.axg_set_binning(self._h, int(mode)))
-
-    def set_fusion(self, mode):
-        self._chk(self._L.axg_set_fusion(self._h, int(mode)))
 
     def set_shard(self, rank, world):
         self._chk(self._L.axg_set_shard(self._h, rank, world))

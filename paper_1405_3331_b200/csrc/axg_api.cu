@@ -60,7 +60,6 @@ struct axg_ctx {
     void* d_cnt = nullptr;
     void* d_scan_state = nullptr;
     int bin_request = AXG_BIN_AUTO;
-    int fuse = AXG_FUSE_OFF;  // axg_set_fusion (checkpoint: the fused kernel is correct but not yet faster)
     bool cnt_dirty = false;   // P1 has counted into cnt and P2 has not consumed (and re-zeroed) it yet
     void* d_src = nullptr;
     void* d_src_id_prefix = nullptr;
@@ -198,11 +197,9 @@ int alloc_particles(axg_ctx* c, uint64_t cap, AxgParams& P, std::vector<void*>& 
     const size_t diff_tiles = n / axg_diffuse_tile() + 2, sort_tiles = n / axg_sort_tile() + 2;
     const size_t sizes[] = {n * 4, n * 4, n * 4, n, n * 4,  // A (SoA)
                             n * 16, n,                      // Brec, Bsp
-                            n * 16,                         // Brec_alt
                             n * 4, n * 4, n * 4, n * 4, n * 4,  // key_pre, skey[2], sidx[2]
-                            diff_tiles * 8, sort_tiles * AXG_RADIX * 8,
-                            (n / AXG_BIG_CELL + 16) * 4};   // big_cells
-    constexpr int NB = 16;
+                            diff_tiles * 8, sort_tiles * AXG_RADIX * 8};
+    constexpr int NB = 14;
     void* ptr[NB];
     for (int i = 0; i < NB; ++i) {
         ptr[i] = dev_alloc(c, sizes[i]);
@@ -216,17 +213,15 @@ int alloc_particles(axg_ctx* c, uint64_t cap, AxgParams& P, std::vector<void*>& 
     P.A = AxgSoA{(float*)ptr[0], (float*)ptr[1], (float*)ptr[2], (uint8_t*)ptr[3], (uint32_t*)ptr[4]};
     P.Brec = (float4*)ptr[5];
     P.Bsp = (uint8_t*)ptr[6];
-    P.Brec_alt = (float4*)ptr[7];
-    P.key_pre = (uint32_t*)ptr[8];
-    P.skey[0] = (uint32_t*)ptr[9]; P.skey[1] = (uint32_t*)ptr[10];
-    P.sidx[0] = (uint32_t*)ptr[11]; P.sidx[1] = (uint32_t*)ptr[12];
-    P.tile_state = (unsigned long long*)ptr[13];
-    P.sort_state = (unsigned long long*)ptr[14];
-    P.big_cells = (uint32_t*)ptr[15];
+    P.key_pre = (uint32_t*)ptr[7];
+    P.skey[0] = (uint32_t*)ptr[8]; P.skey[1] = (uint32_t*)ptr[9];
+    P.sidx[0] = (uint32_t*)ptr[10]; P.sidx[1] = (uint32_t*)ptr[11];
+    P.tile_state = (unsigned long long*)ptr[12];
+    P.sort_state = (unsigned long long*)ptr[13];
     P.capacity = (uint32_t)cap;
     // look-back words must not alias a live epoch: zero them (epoch 0 words with flag 0 = not ready)
+    CU(c, cudaMemsetAsync(ptr[12], 0, sizes[12], c->stream));
     CU(c, cudaMemsetAsync(ptr[13], 0, sizes[13], c->stream));
-    CU(c, cudaMemsetAsync(ptr[14], 0, sizes[14], c->stream));
     return AXG_OK;
 }
 
@@ -390,10 +385,9 @@ int enqueue_phases(axg_ctx* c, uint32_t mask, Prof& prof, bool overlap = false) 
             axg_launch_cell_scan(P, N_SM * 4, s);
             prof.mark(AXG_K_PLACE);
             axg_launch_place(P, N_SM * 8, s);
-            axg_launch_sort_big_cells(P, s);  // timed with k_place
             prof.mark(AXG_K_SETTLE);
             axg_launch_settle(P, N_SM * 8, s);
-            launches += 4;
+            launches += 3;
             c->cnt_dirty = false;
         } else {
             prof.mark(AXG_K_SORT);
@@ -434,60 +428,6 @@ int enqueue_phases(axg_ctx* c, uint32_t mask, Prof& prof, bool overlap = false) 
         launches += 1;
     }
     return launches;
-}
-
-// n whole steps with count binning, P2b/P2c of step t fused into P1 of step t+1 (k_diffuse<true>, axg_set_fusion):
-//   k_diffuse | scan, place, [sense, advance] | k_settle_diffuse | scan, place, [sense, advance] | ... | k_settle
-// The cone kernels need cell_lo and the slot list only (k_sense reads the species from the slot values), so with
-// `overlap` they run on the side stream beside the next fused kernel; the next scan waits for them.
-int enqueue_steps_fused(axg_ctx* c, uint32_t n, Prof& prof, bool overlap) {
-    AxgParams& P = c->P;
-    cudaStream_t s = c->stream;
-    int launches = 0;
-    if (c->cnt_dirty) cudaMemsetAsync(c->d_cnt, 0, c->cells_padded() * sizeof(uint32_t), s);
-    P.materialize = c->fuse == AXG_FUSE_MATERIALIZE ? 1 : 0;
-    for (uint32_t i = 0; i < n; ++i) {
-        if (i == 0) {
-            prof.mark(AXG_K_DIFFUSE);
-            axg_launch_diffuse(P, N_SM * 4, s);
-        } else {
-            prof.mark(AXG_K_SETTLE_DIFFUSE);
-            axg_launch_settle_diffuse(P, N_SM * 3, s);  // reads Brec (step i-1), writes Brec_alt (step i)
-            std::swap(P.Brec, P.Brec_alt);
-        }
-        if (overlap && c->adv_pending) cudaStreamWaitEvent(s, c->ev_adv, 0);  // P3 of step i-1 reads cell_lo / slots
-        prof.mark(AXG_K_SCAN);
-        axg_launch_cell_scan(P, N_SM * 4, s);
-        prof.mark(AXG_K_PLACE);
-        axg_launch_place(P, N_SM * 8, s);
-        axg_launch_sort_big_cells(P, s);  // timed with k_place
-        launches += 4;
-        cudaStream_t sc = s;
-        if (overlap) {
-            cudaEventRecord(c->ev_bin, s);
-            cudaStreamWaitEvent(c->side, c->ev_bin, 0);
-            sc = c->side;
-        }
-        if (P.n_cones) {
-            prof.mark(AXG_K_SENSE);
-            axg_launch_sense(P, sc);
-            prof.mark(AXG_K_ADVANCE);
-            axg_launch_advance(P, 1, sc);  // O10 rides in its last block
-            launches += 2;
-        } else {
-            prof.mark(AXG_K_COMMIT);
-            axg_launch_commit(P, 1, s);
-            launches += 1;
-        }
-        if (overlap) {
-            cudaEventRecord(c->ev_adv, c->side);
-            c->adv_pending = true;
-        }
-    }
-    prof.mark(AXG_K_SETTLE);  // the sorted SoA, keys and permutation of the last step, for axg_read_state and the next call
-    axg_launch_settle(P, N_SM * 8, s);
-    c->cnt_dirty = false;
-    return launches + 1;
 }
 
 void finish_prof(axg_ctx* c, Prof& prof) {
@@ -594,13 +534,6 @@ AXG_API int axg_set_binning(axg_ctx* c, int mode) {
     if (c->cnt_dirty) return fail(c, AXG_ESTATE, "a step is half done (P1 without P2)");
     c->bin_request = mode;
     return c->particles_allocated ? resolve_binning(c) : AXG_OK;
-}
-
-AXG_API int axg_set_fusion(axg_ctx* c, int mode) {
-    if (!c || (mode != AXG_FUSE_OFF && mode != AXG_FUSE_ON && mode != AXG_FUSE_MATERIALIZE))
-        return fail(c, AXG_EINVAL, "bad fusion mode");
-    c->fuse = mode;
-    return AXG_OK;
 }
 
 AXG_API int axg_add_source(axg_ctx* c, float x, float y, float z, uint8_t species, int8_t polarity, uint32_t rate) {
@@ -763,10 +696,7 @@ AXG_API int axg_step(axg_ctx* c, uint32_t n) {
         CU(c, cudaEventCreateWithFlags(&c->ev_adv, cudaEventDisableTiming));
     }
     CU(c, cudaEventRecord(c->ev0, c->stream));
-    if (c->fuse != AXG_FUSE_OFF && c->P.bin_mode == AXG_BIN_COUNT_D && n > 1)
-        launches += enqueue_steps_fused(c, n, prof, overlap);
-    else
-        for (uint32_t i = 0; i < n; ++i) launches += enqueue_phases(c, AXG_PHASE_ALL, prof, overlap);
+    for (uint32_t i = 0; i < n; ++i) launches += enqueue_phases(c, AXG_PHASE_ALL, prof, overlap);
     if (c->adv_pending) {  // join: the ctx stream waits for the last step's cones
         CU(c, cudaStreamWaitEvent(c->stream, c->ev_adv, 0));
         c->adv_pending = false;

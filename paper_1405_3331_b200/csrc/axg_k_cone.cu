@@ -13,11 +13,6 @@ __global__ void __launch_bounds__(256) k_sense(const AxgParams p) {
     const int lane = threadIdx.x & 31;
     const uint32_t warps_total = (gridDim.x * blockDim.x) >> 5;
     const uint32_t* __restrict__ cell_lo = p.cell_lo;
-    // count binning: the species of a cell's members are read from the slot list of k_place (top two bits of the sort
-    // value; the order inside a cell does not matter for a sum), so that P3 needs nothing of k_settle and may run
-    // beside the fused settle + diffuse kernel of the next step.  Radix binning: the sorted species column.
-    const bool from_slots = p.bin_mode == AXG_BIN_COUNT_D;
-    const uint32_t* __restrict__ slot = p.sidx[p.final_buf ^ 1];
     for (uint32_t c = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; c < p.n_cones; c += warps_total) {
         if (p.cone_state[c] != 0) {  // frozen cones skip P3..P5 (reading A-16)
             if (p.sharded && lane < 16) p.sense[(size_t)c * 16 + lane] = 0;
@@ -46,7 +41,7 @@ __global__ void __launch_bounds__(256) k_sense(const AxgParams p) {
                     }
             } else {
                 for (uint32_t j = a; j < b; ++j) {
-                    const int sp = from_slots ? (int)(__ldg(slot + j) >> 30) : (int)__ldg(p.A.species + j);
+                    const int sp = (int)__ldg(p.A.species + j);
 #pragma unroll
                     for (int s = 0; s < AXG_MAX_SPECIES_D; ++s)
                         if (s == sp) { acc[s][0] += 1; acc[s][1] += dx; acc[s][2] += dy; acc[s][3] += dz; }

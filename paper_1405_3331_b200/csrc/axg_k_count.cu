@@ -45,16 +45,6 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_cell_scan(const AxgParams p) {
         uint4 v[SCAN_ITEMS / 4];
 #pragma unroll
         for (int k = 0; k < SCAN_ITEMS / 4; ++k) v[k] = reinterpret_cast<const uint4*>(p.cnt)[at4 + 32 * k];
-        // crowded cells (next to a source) are listed for k_sort_big_cells; element e of cnt counts cell e - 1
-#pragma unroll
-        for (int k = 0; k < SCAN_ITEMS / 4; ++k)
-            if (max(max(v[k].x, v[k].y), max(v[k].z, v[k].w)) > AXG_BIG_CELL) {
-                const uint32_t e0 = (uint32_t)((at4 + 32 * k) * 4);
-                const uint32_t c4[4] = {v[k].x, v[k].y, v[k].z, v[k].w};
-#pragma unroll
-                for (int a = 0; a < 4; ++a)
-                    if (c4[a] > AXG_BIG_CELL) p.big_cells[atomicAdd(&dev->n_big, 1u)] = e0 + a - 1u;
-            }
         uint32_t pre[SCAN_ITEMS / 4];  // particles before my 4 cells of chunk k, inside the warp's segment
         uint32_t carry = 0u;
 #pragma unroll
@@ -138,58 +128,6 @@ __global__ void __launch_bounds__(PLACE_THREADS) k_place(const AxgParams p) {
     }
 }
 
-// ---- crowded cells: sort the slot range by pre-sort index, so that rank = position ------------------------------------
-// The quadratic rank loop of k_settle is right for the ~1.6 members of a typical cell and hopeless for the hundreds
-// to thousands of a source cell (all newborns of a source share its cell).  k_cell_scan lists the cells with more than
-// AXG_BIG_CELL members; one block per listed cell sorts slot[lo, hi) by the index bits with a bitonic network (the
-// all-ascending form: partner i ^ (2k - 1) in the first step of a merge, i ^ j after it, so virtual +inf padding
-// beyond the range never moves), in shared memory when the cell fits, in place in global memory otherwise.
-constexpr int BIG_THREADS = 256;
-constexpr uint32_t BIG_SMEM = 8192;
-
-__device__ __forceinline__ void bitonic_sort_masked(uint32_t* a, uint32_t m) {
-    uint32_t np2 = 1u;
-    while (np2 < m) np2 <<= 1;
-    for (uint32_t k = 2u; k <= np2; k <<= 1) {
-        for (uint32_t j = k >> 1; j > 0u; j >>= 1) {
-            const uint32_t flip = (j == (k >> 1)) ? (k - 1u) : j;
-            for (uint32_t i = threadIdx.x; i < np2; i += BIG_THREADS) {
-                const uint32_t l = i ^ flip;
-                if (l > i && l < m) {  // l >= m: the partner is +inf padding, nothing to exchange
-                    const uint32_t x = a[i], y = a[l];
-                    if ((x & AXG_IDX_MASK) > (y & AXG_IDX_MASK)) { a[i] = y; a[l] = x; }
-                }
-            }
-            __syncthreads();
-        }
-    }
-}
-
-__global__ void __launch_bounds__(BIG_THREADS) k_sort_big_cells(const AxgParams p) {
-    __shared__ uint32_t s_a[BIG_SMEM];
-    AxgDev* dev = p.dev;
-    const uint32_t n_big = dev->n_big;
-    uint32_t* slot = p.sidx[p.final_buf ^ 1];
-    for (uint32_t b = blockIdx.x; b < n_big; b += gridDim.x) {
-        const uint32_t c = p.big_cells[b];
-        const uint32_t lo = p.cell_lo[c], m = p.cell_lo[c + 1u] - lo;
-        if (m <= BIG_SMEM) {
-            for (uint32_t i = threadIdx.x; i < m; i += BIG_THREADS) s_a[i] = slot[lo + i];
-            __syncthreads();
-            bitonic_sort_masked(s_a, m);
-            for (uint32_t i = threadIdx.x; i < m; i += BIG_THREADS) slot[lo + i] = s_a[i];
-            __syncthreads();
-        } else {
-            __syncthreads();
-            bitonic_sort_masked(slot + lo, m);  // block-local: __syncthreads orders the global accesses
-        }
-    }
-    if (axg_last_block(dev) && threadIdx.x == 0) {
-        dev->done = 0u;
-        dev->n_big = 0u;
-    }
-}
-
 // ---- rank inside the cell by pre-sort index, then O5: A[cell_lo + rank] = B[index] -------------------------------
 constexpr int SETTLE_THREADS = 256;
 constexpr int SETTLE_ITEMS = 1;  // warp-striped (item i of lane l is slot base + 32 i + l).  Measured at C3: 1 item and
@@ -228,9 +166,7 @@ __global__ void __launch_bounds__(SETTLE_THREADS, 8) k_settle(const AxgParams p)
             const uint32_t k = axg_cell_key(p, r[i].x, r[i].y, r[i].z);
             const uint32_t lo = __ldg(cell_lo + k), hi = __ldg(cell_lo + k + 1u);
             uint32_t rank = 0u;  // members of my cell with a smaller pre-sort index (reading A-9: ties keep that order)
-            if (hi - lo > AXG_BIG_CELL)  // crowded cell: k_sort_big_cells has sorted its slots, rank = position
-                rank = j - lo;
-            else if (hi - lo > 1u)  // alone in the cell (the common case): nothing to rank against
+            if (hi - lo > 1u)  // alone in the cell (the common case): nothing to rank against
                 for (uint32_t q = lo; q < hi; ++q) rank += ((__ldg(slot + q) & AXG_IDX_MASK) < idx) ? 1u : 0u;
             const uint32_t dst = lo + rank;
             p.A.x[dst] = r[i].x;
@@ -248,5 +184,4 @@ __global__ void __launch_bounds__(SETTLE_THREADS, 8) k_settle(const AxgParams p)
 
 void axg_launch_cell_scan(const AxgParams& p, int grid, cudaStream_t s) { k_cell_scan<<<grid, SCAN_THREADS, 0, s>>>(p); }
 void axg_launch_place(const AxgParams& p, int grid, cudaStream_t s) { k_place<<<grid, PLACE_THREADS, 0, s>>>(p); }
-void axg_launch_sort_big_cells(const AxgParams& p, cudaStream_t s) { k_sort_big_cells<<<64, BIG_THREADS, 0, s>>>(p); }
 void axg_launch_settle(const AxgParams& p, int grid, cudaStream_t s) { k_settle<<<grid, SETTLE_THREADS, 0, s>>>(p); }

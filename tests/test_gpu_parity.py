@@ -185,3 +185,28 @@ def test_errors_and_capacity(axg):
         axg.Axg((0, 8, 8), 0.5, 4, 2.0, 0.25, 0.1, 1)
     with pytest.raises(axg.AxgError):
         axg.Axg((8, 8, 8), 0.5, 4, 9.0, 0.25, 0.1, 1)
+
+
+@pytest.mark.parametrize("n", [20_000, 90_000])
+def test_binning_crowded_cells(axg, n):
+    """80 % of the particles inside a 1.5-cell cube (a source cell holds hundreds to thousands of members in the coarse
+    pre-run): cells of several thousand members, i.e. the quadratic rank loop of count binning and long equal-key runs
+    in the radix passes, against std::stable_sort, bit for bit."""
+    grid = (12, 10, 9)
+    g = pu.new_axg(axg, grid, 0.5, 1, 2.0, 0.25, 0.1, 3)
+    o = axo.Oracle(grid, 0.5, 1, 2.0, 0.25, 0.1, 3)
+    g.set_capacity(n + 16, 4)
+    o.set_capacity(n + 16, 4)
+    x, y, z, sp, ids = W.random_particles(5, n, grid, n_species=2)
+    k = int(n * 0.8)
+    for a, c in zip((x, y, z), (5.0, 4.0, 3.0)):
+        a[:k] = c + (a[:k] - np.floor(a[:k])) * 1.5
+    for s in (g, o):
+        s.load_particles(x, y, z, sp, ids, next_id=n, step=0)
+    g.step_phase(axg.PHASE_BIN)
+    o.step_phase(axo.PHASE_BIN)
+    occupancy = o.read_state("CELL_END").astype(np.int64) - o.read_state("CELL_START")
+    assert occupancy.max() > (8192 if n > 50_000 else 2048)
+    compare_binning(g, o)
+    g.close()
+    o.close()
