@@ -60,6 +60,7 @@ struct axg_ctx {
     void* d_cnt = nullptr;
     void* d_scan_state = nullptr;
     int bin_request = AXG_BIN_AUTO;
+    bool b_chunked = false;   // the pre-sort array is in the chunked layout of k_diffuse_chunked (count binning)
     bool cnt_dirty = false;   // P1 has counted into cnt and P2 has not consumed (and re-zeroed) it yet
     void* d_src = nullptr;
     void* d_src_id_prefix = nullptr;
@@ -192,14 +193,15 @@ void free_particles(axg_ctx* c) {
 
 // fills P.A, P.B, keys, look-back words for `cap` particles
 int alloc_particles(axg_ctx* c, uint64_t cap, AxgParams& P, std::vector<void*>& bufs) {
-    const size_t pad = 64;  // tail padding so that ragged tiles may over-read harmlessly
+    const size_t pad = 256;  // tail padding: ragged tiles may over-read harmlessly; the chunked layout rounds up to 128
     const size_t n = (size_t)cap + pad;
     const size_t diff_tiles = n / axg_diffuse_tile() + 2, sort_tiles = n / axg_sort_tile() + 2;
     const size_t sizes[] = {n * 4, n * 4, n * 4, n, n * 4,  // A (SoA)
                             n * 16, n,                      // Brec, Bsp
                             n * 4, n * 4, n * 4, n * 4, n * 4,  // key_pre, skey[2], sidx[2]
-                            diff_tiles * 8, sort_tiles * AXG_RADIX * 8};
-    constexpr int NB = 14;
+                            diff_tiles * 8, sort_tiles * AXG_RADIX * 8,
+                            (n / AXG_CHUNK + 4) * 4, (n / AXG_CHUNK + 4) * 4};  // chunk_cnt, chunk_base
+    constexpr int NB = 16;
     void* ptr[NB];
     for (int i = 0; i < NB; ++i) {
         ptr[i] = dev_alloc(c, sizes[i]);
@@ -218,6 +220,8 @@ int alloc_particles(axg_ctx* c, uint64_t cap, AxgParams& P, std::vector<void*>& 
     P.sidx[0] = (uint32_t*)ptr[10]; P.sidx[1] = (uint32_t*)ptr[11];
     P.tile_state = (unsigned long long*)ptr[12];
     P.sort_state = (unsigned long long*)ptr[13];
+    P.chunk_cnt = (uint32_t*)ptr[14];
+    P.chunk_base = (uint32_t*)ptr[15];
     P.capacity = (uint32_t)cap;
     // look-back words must not alias a live epoch: zero them (epoch 0 words with flag 0 = not ready)
     CU(c, cudaMemsetAsync(ptr[12], 0, sizes[12], c->stream));
@@ -369,6 +373,7 @@ int enqueue_phases(axg_ctx* c, uint32_t mask, Prof& prof, bool overlap = false) 
         axg_launch_diffuse(P, N_SM * 4, s);  // its last block emits and closes P1
         launches += 1;
         c->cnt_dirty = count_mode;
+        c->b_chunked = count_mode;
     }
     if (mask & AXG_PHASE_BIN) {
         // the previous step's P3 (side stream) still reads cell_lo and the species column that P2 rewrites
@@ -379,6 +384,7 @@ int enqueue_phases(axg_ctx* c, uint32_t mask, Prof& prof, bool overlap = false) 
             axg_launch_rekey(P, N_SM * 8, s);
             axg_launch_emit(P, 0, s);
             launches += 2;
+            c->b_chunked = count_mode;
         }
         if (count_mode) {
             prof.mark(AXG_K_SCAN);
@@ -841,7 +847,7 @@ AXG_API int axg_read_state(axg_ctx* c, uint32_t field, void* dst, size_t dst_byt
         case AXG_KEYS_SORTED: return copy_out(c, have_p ? P.skey[P.final_buf] : nullptr, nB, 4, dst, dst_bytes, n_elems);
         case AXG_PERM:
             return export_out(c, nB, 4, dst, dst_bytes, n_elems,
-                              [&](void* t) { axg_launch_perm_export(P, (uint32_t*)t, c->stream); });
+                              [&](void* t) { axg_launch_perm_export(P, c->b_chunked ? 1 : 0, (uint32_t*)t, c->stream); });
         case AXG_CELL_START:
             return export_out(c, c->cells(), 4, dst, dst_bytes, n_elems,
                               [&](void* t) { axg_launch_cell_export(P, (uint32_t*)t, nullptr, c->stream); });
@@ -868,10 +874,14 @@ AXG_API int axg_read_state(axg_ctx* c, uint32_t field, void* dst, size_t dst_byt
         case AXG_PRE_ID: {
             const int comp = field == AXG_PRE_ID ? 3 : (int)(field - AXG_PRE_X);
             return export_out(c, nB, 4, dst, dst_bytes, n_elems,
-                              [&](void* t) { axg_launch_pre_export(P, comp, (uint32_t*)t, c->stream); });
+                              [&](void* t) { axg_launch_pre_export(P, comp, c->b_chunked ? 1 : 0, t, c->stream); });
         }
-        case AXG_PRE_SPECIES: return copy_out(c, P.Bsp, nB, 1, dst, dst_bytes, n_elems);
-        case AXG_PRE_KEY: return copy_out(c, P.key_pre, nB, 4, dst, dst_bytes, n_elems);
+        case AXG_PRE_SPECIES:
+            return export_out(c, nB, 1, dst, dst_bytes, n_elems,
+                              [&](void* t) { axg_launch_pre_export(P, 5, c->b_chunked ? 1 : 0, t, c->stream); });
+        case AXG_PRE_KEY:
+            return export_out(c, nB, 4, dst, dst_bytes, n_elems,
+                              [&](void* t) { axg_launch_pre_export(P, 4, c->b_chunked ? 1 : 0, t, c->stream); });
         default: return fail(c, AXG_EINVAL, "unknown field");
     }
 }

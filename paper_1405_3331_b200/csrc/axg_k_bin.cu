@@ -149,19 +149,63 @@ __global__ void __launch_bounds__(BIN_THREADS) k_reorder4(const AxgParams p) {
     }
 }
 
-// read path: one column of the pre-sort records (0..2 = x, y, z as f32 bits, 3 = id), and the permutation without
-// the species bits
-__global__ void k_pre_export(const AxgParams p, int component, uint32_t* __restrict__ dst) {
-    const uint32_t n = p.dev->n_live;
-    const uint32_t* __restrict__ src = reinterpret_cast<const uint32_t*>(p.Brec);
-    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
-        dst[i] = src[(size_t)i * 4 + component];
+// ---- read path of the pre-sort array and the permutation ----------------------------------------------------------
+// Radix binning keeps the pre-sort array dense.  Count binning keeps it in the chunked layout of k_diffuse_chunked
+// (holes at the end of every 128-row chunk); the ABI's pre-sort index of physical row o is chunk_base[o / 128] + o % 128
+// (newborns: survivors + offset), with chunk_base = exclusive scan of chunk_cnt, computed here on demand.
+__global__ void __launch_bounds__(1024) k_chunk_scan(const AxgParams p) {
+    __shared__ uint32_t s_sum[1024];
+    const uint32_t n_chunks = p.dev->n_phys / AXG_CHUNK;
+    const uint32_t per = (n_chunks + 1023u) / 1024u;
+    const uint32_t lo = min(threadIdx.x * per, n_chunks), hi = min(lo + per, n_chunks);
+    uint32_t sum = 0u;
+    for (uint32_t q = lo; q < hi; ++q) sum += p.chunk_cnt[q];
+    s_sum[threadIdx.x] = sum;
+    __syncthreads();
+    for (uint32_t d = 1u; d < 1024u; d <<= 1) {  // Hillis-Steele inclusive scan of the 1024 partial sums
+        const uint32_t v = threadIdx.x >= d ? s_sum[threadIdx.x - d] : 0u;
+        __syncthreads();
+        s_sum[threadIdx.x] += v;
+        __syncthreads();
+    }
+    uint32_t run = s_sum[threadIdx.x] - sum;
+    for (uint32_t q = lo; q < hi; ++q) {
+        p.chunk_base[q] = run;
+        run += p.chunk_cnt[q];
+    }
 }
-__global__ void k_perm_export(const AxgParams p, uint32_t* __restrict__ dst) {
+
+__device__ __forceinline__ bool axg_is_hole(const AxgParams& p, uint32_t o, uint32_t n_phys) {
+    return o < n_phys && (o % AXG_CHUNK) >= p.chunk_cnt[o / AXG_CHUNK];
+}
+__device__ __forceinline__ uint32_t axg_dense_index(const AxgParams& p, uint32_t o, uint32_t n_phys, uint32_t n_surv) {
+    return o >= n_phys ? n_surv + (o - n_phys) : p.chunk_base[o / AXG_CHUNK] + (o % AXG_CHUNK);
+}
+
+// one column of the pre-sort array in dense order: component 0..2 = x, y, z (f32 bits), 3 = id, 4 = key (all to
+// uint32 dst), 5 = species (to uint8 dst)
+__global__ void k_pre_export(const AxgParams p, int component, int chunked, void* __restrict__ dst) {
+    const uint32_t n_live = p.dev->n_live;
+    const uint32_t n_phys = chunked ? p.dev->n_phys : 0u, n_rows = chunked ? p.dev->n_pp : n_live;
+    const uint32_t n_surv = n_live - (n_rows - n_phys);
+    const uint32_t* __restrict__ rec = reinterpret_cast<const uint32_t*>(p.Brec);
+    for (uint32_t o = blockIdx.x * blockDim.x + threadIdx.x; o < n_rows; o += gridDim.x * blockDim.x) {
+        if (chunked && axg_is_hole(p, o, n_phys)) continue;
+        const uint32_t i = chunked ? axg_dense_index(p, o, n_phys, n_surv) : o;
+        if (component < 4) static_cast<uint32_t*>(dst)[i] = rec[(size_t)o * 4 + component];
+        else if (component == 4) static_cast<uint32_t*>(dst)[i] = p.key_pre[o];
+        else static_cast<uint8_t*>(dst)[i] = p.Bsp[o];
+    }
+}
+// the permutation (sorted slot -> pre-sort index) without the species bits
+__global__ void k_perm_export(const AxgParams p, int chunked, uint32_t* __restrict__ dst) {
     const uint32_t n = p.dev->n_live;
+    const uint32_t n_phys = p.dev->n_phys, n_surv = n - (p.dev->n_pp - n_phys);
     const uint32_t* __restrict__ src = p.sidx[p.final_buf];
-    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
-        dst[i] = src[i] & AXG_IDX_MASK;
+    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const uint32_t o = src[i] & AXG_IDX_MASK;
+        dst[i] = chunked ? axg_dense_index(p, o, n_phys, n_surv) : o;
+    }
 }
 
 // cellStart / cellEnd in the paper's convention from cell_lo (read path only)
@@ -180,11 +224,13 @@ void axg_launch_reorder(const AxgParams& p, int grid, int wide, cudaStream_t s) 
     if (wide) k_reorder4<<<grid, BIN_THREADS, 0, s>>>(p); else k_reorder<<<grid, BIN_THREADS, 0, s>>>(p);
 }
 
-void axg_launch_pre_export(const AxgParams& p, int component, uint32_t* dst, cudaStream_t s) {
-    k_pre_export<<<148 * 8, 256, 0, s>>>(p, component, dst);
+void axg_launch_pre_export(const AxgParams& p, int component, int chunked, void* dst, cudaStream_t s) {
+    if (chunked) k_chunk_scan<<<1, 1024, 0, s>>>(p);
+    k_pre_export<<<148 * 8, 256, 0, s>>>(p, component, chunked, dst);
 }
-void axg_launch_perm_export(const AxgParams& p, uint32_t* dst, cudaStream_t s) {
-    k_perm_export<<<148 * 8, 256, 0, s>>>(p, dst);
+void axg_launch_perm_export(const AxgParams& p, int chunked, uint32_t* dst, cudaStream_t s) {
+    if (chunked) k_chunk_scan<<<1, 1024, 0, s>>>(p);
+    k_perm_export<<<148 * 8, 256, 0, s>>>(p, chunked, dst);
 }
 
 void axg_launch_cell_export(const AxgParams& p, uint32_t* start, uint32_t* end, cudaStream_t s) {

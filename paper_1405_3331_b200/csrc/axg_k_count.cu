@@ -115,12 +115,15 @@ __device__ __forceinline__ uint32_t take_slot(uint32_t* __restrict__ cell_lo, ui
 }
 
 __global__ void __launch_bounds__(PLACE_THREADS) k_place(const AxgParams p) {
-    const uint32_t n = p.dev->n_live;
+    // B is in the chunked layout of k_diffuse_chunked: every physical row below n_pp is visited, the holes at the end
+    // of each chunk are skipped, and the slot value is the PHYSICAL row (it orders the rows like the dense index)
+    const uint32_t n_phys = p.dev->n_phys, n_pp = p.dev->n_pp;
     uint32_t* __restrict__ slot = p.sidx[p.final_buf ^ 1];
     uint32_t* __restrict__ cell_lo = p.cell_lo;
     // one particle per thread: measured faster than four per thread with 128-bit loads (0.176 vs 0.213 ms at C3) -- the
     // kernel is bound by L2 transactions (one atomic + one scattered 4-byte store each) and wants many warps in flight
-    for (uint32_t o = blockIdx.x * PLACE_THREADS + threadIdx.x; o < n; o += gridDim.x * PLACE_THREADS) {
+    for (uint32_t o = blockIdx.x * PLACE_THREADS + threadIdx.x; o < n_pp; o += gridDim.x * PLACE_THREADS) {
+        if (o < n_phys && (o % AXG_CHUNK) >= __ldg(p.chunk_cnt + o / AXG_CHUNK)) continue;  // a hole
         const uint32_t k = __ldg(p.key_pre + o);
         const uint32_t sp = __ldg(p.Bsp + o);
         // bumping the cursor hands out the slots of the cell in the arbitrary order of the atomics

@@ -37,9 +37,14 @@ __device__ void emit_and_close(const AxgParams& p, int do_emit, uint32_t (*s_his
     AxgDev* dev = p.dev;
     const int tid = threadIdx.x, nthr = blockDim.x;
     const uint32_t n_in = dev->n_live;
-    const uint32_t n_surv = do_emit ? (n_in ? dev->n_surv : 0u) : n_in;
+    // volatile: written by other blocks of this kernel; the line may sit in this SM's L1 from the read of n_live
+    const uint32_t n_surv = do_emit ? (n_in ? *(volatile uint32_t*)&dev->n_surv : 0u) : n_in;
     const uint32_t next_id = dev->next_id;
-    const bool fits = (unsigned long long)n_surv + p.e_owned <= (unsigned long long)p.capacity;
+    // count binning: B is in the chunked layout, the newborns follow the last chunk (AxgDev::n_phys)
+    const bool chunked = p.bin_mode == AXG_BIN_COUNT_D;
+    const uint32_t n_phys = chunked ? ((n_in + AXG_CHUNK - 1u) / AXG_CHUNK) * AXG_CHUNK : n_surv;
+    const bool fits = (unsigned long long)n_surv + p.e_owned <= (unsigned long long)p.capacity &&
+                      (unsigned long long)n_phys + p.e_owned <= (unsigned long long)p.capacity + AXG_CHUNK;
     __syncthreads();
     for (int i = tid; i < AXG_MAX_PASSES * AXG_RADIX; i += nthr) (&s_hist[0][0])[i] = 0u;
     __syncthreads();
@@ -53,7 +58,7 @@ __device__ void emit_and_close(const AxgParams& p, int do_emit, uint32_t (*s_his
             }
             const uint32_t s = lo, j = e - p.src_emit_prefix[s];
             const AxgSourceDev sd = p.src[s];
-            const uint32_t o = n_surv + e;
+            const uint32_t o = n_phys + e;
             const uint32_t key = axg_cell_key(p, sd.x, sd.y, sd.z);
             p.Brec[o] = make_float4(sd.x, sd.y, sd.z, __uint_as_float(next_id + p.src_id_prefix[s] + j));
             p.Bsp[o] = (uint8_t)(sd.species_polarity & 0xffu);
@@ -91,10 +96,18 @@ __device__ void emit_and_close(const AxgParams& p, int do_emit, uint32_t (*s_his
             __syncthreads();
         }
     }
+    if (tid == 0 && !do_emit) {  // harness path after k_rekey: B is dense, which is a valid chunked layout too
+        dev->n_surv = 0u;
+        dev->n_phys = n_phys;
+        dev->n_pp = n_phys;
+    }
     if (tid == 0 && do_emit) {
         dev->pstep += 1u;  // P1 of step t is done: the next k_diffuse draws from (id, t + 1)
         if (!fits) atomicOr(&dev->err, 1u);
         dev->n_live = fits ? n_surv + p.e_owned : n_surv;
+        dev->n_surv = 0u;  // k_diffuse_chunked accumulates into it
+        dev->n_phys = n_phys;
+        dev->n_pp = n_phys + (do_emit && fits ? p.e_owned : 0u);
         dev->next_id = next_id + p.e_total;
         dev->emitted += fits ? p.e_owned : 0u;
         dev->absorbed += n_in - n_surv;
@@ -246,6 +259,80 @@ __global__ void __launch_bounds__(DIFF_THREADS, 4) k_diffuse(const AxgParams p) 
     }
 }
 
+// ---- P1 for count binning: compaction inside chunks, no chain ------------------------------------------------------
+// The chained kernel above produces a DENSE pre-sort array, which makes every tile wait for the survivor count of every
+// tile before it: all blocks march in lock-step, and at C3 a third of the issue slots go to the barriers around the
+// look-back and to the burst of stores after it (profiles/).  Count binning never reads the pre-sort array
+// sequentially by index -- k_place only needs to visit every row once, k_settle gathers by position -- so here each
+// warp compacts its own chunk of 128 rows in place: chunk q's survivors go to B[128 q .. 128 q + chunk_cnt[q]), in
+// input order (ballot / popc ranks, reading A-6), straight from registers.  No shared memory, no block barrier, no
+// look-back.  The position of a row in this layout orders the rows exactly as the dense index would, so the stable
+// order of P2 is unchanged; the dense index itself (the permutation the ABI reports) is chunk_base + offset, computed
+// by the export kernels only.
+__global__ void __launch_bounds__(DIFF_THREADS, 4) k_diffuse_chunked(const AxgParams p) {
+    __shared__ uint32_t s_hist[AXG_MAX_PASSES][AXG_RADIX];  // scratch of emit_and_close only
+    __shared__ uint32_t s_surv;
+    AxgDev* dev = p.dev;
+    const uint32_t n_in = dev->n_live, t = dev->pstep;
+    const uint32_t n_chunks = (n_in + AXG_CHUNK - 1u) / AXG_CHUNK;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const uint32_t lt = axg_lanemask_lt();
+    const AxgRoundKeys rk = axg_round_keys(p.seed_lo, p.seed_hi);
+    static_assert(32 * DIFF_ITEMS == AXG_CHUNK, "one warp trip = one chunk");
+    if (tid == 0) s_surv = 0u;
+    __syncthreads();
+
+    uint32_t mine = 0u;  // survivors of my warp's chunks (lane 0)
+    const uint32_t warps_total = (gridDim.x * DIFF_THREADS) >> 5;
+    for (uint32_t chunk = (blockIdx.x * DIFF_THREADS + tid) >> 5; chunk < n_chunks; chunk += warps_total) {
+        const uint32_t first = chunk * AXG_CHUNK + lane;
+        float x[DIFF_ITEMS], y[DIFF_ITEMS], z[DIFF_ITEMS];
+        uint32_t id[DIFF_ITEMS], sp[DIFF_ITEMS];
+#pragma unroll
+        for (int i = 0; i < DIFF_ITEMS; ++i) {
+            const uint32_t g = first + i * 32;
+            const bool v = g < n_in;
+            x[i] = v ? __ldg(p.A.x + g) : -1.0f;
+            y[i] = v ? __ldg(p.A.y + g) : -1.0f;
+            z[i] = v ? __ldg(p.A.z + g) : -1.0f;
+            id[i] = v ? __ldg(p.A.id + g) : 0u;
+            sp[i] = v ? (uint32_t)__ldg(p.A.species + g) : 0u;
+        }
+        uint32_t out = chunk * AXG_CHUNK;
+#pragma unroll
+        for (int i = 0; i < DIFF_ITEMS; ++i) {
+            const bool v = (first + i * 32) < n_in;
+            float z0, z1, z2;
+            axg_normals3(id[i], t, 0u, rk, z0, z1, z2);                       // O1
+            const float xn = fmaf(p.sigma, z0, x[i]), yn = fmaf(p.sigma, z1, y[i]), zn = fmaf(p.sigma, z2, z[i]);
+            const bool in = xn >= 0.0f && xn < p.fnx && yn >= 0.0f && yn < p.fny && zn >= 0.0f && zn < p.fnz;  // P1b
+            const uint32_t b = __ballot_sync(0xffffffffu, v && in);
+            if (v && in) {                                                     // P1d + P2a
+                const uint32_t o = out + __popc(b & lt);
+                const uint32_t key = axg_cell_key(p, xn, yn, zn);
+                p.Brec[o] = make_float4(xn, yn, zn, __uint_as_float(id[i]));
+                p.Bsp[o] = (uint8_t)sp[i];
+                p.key_pre[o] = key;
+                atomicAdd(p.cnt + key + 1u, 1u);  // fire-and-forget RED (see tally)
+            }
+            out += __popc(b);
+        }
+        if (lane == 0) {
+            const uint32_t c = out - chunk * AXG_CHUNK;
+            p.chunk_cnt[chunk] = c;
+            mine += c;
+        }
+    }
+    if (lane == 0 && mine) atomicAdd(&s_surv, mine);
+    __syncthreads();
+    if (tid == 0 && s_surv) atomicAdd(&dev->n_surv, s_surv);
+    if (axg_last_block(dev)) {  // every block's survivors, keys and counts are visible here
+        if (tid == 0) dev->done = 0u;
+        __threadfence();
+        emit_and_close(p, 1, s_hist);
+    }
+}
+
 // harness path: B = A, key_pre = key(A), histograms.  No RNG, no compaction.
 __global__ void __launch_bounds__(256) k_rekey(const AxgParams p) {
     __shared__ uint32_t s_hist[AXG_MAX_PASSES][AXG_RADIX];
@@ -259,6 +346,7 @@ __global__ void __launch_bounds__(256) k_rekey(const AxgParams p) {
         p.Brec[g] = make_float4(x, y, z, __uint_as_float(p.A.id[g]));
         p.Bsp[g] = p.A.species[g];
         p.key_pre[g] = key;
+        if (p.bin_mode == AXG_BIN_COUNT_D && (g % AXG_CHUNK) == 0u) p.chunk_cnt[g / AXG_CHUNK] = min(AXG_CHUNK, n - g);
         tally(p, s_hist, key);
     }
     __syncthreads();
@@ -278,6 +366,9 @@ __global__ void __launch_bounds__(EMIT_THREADS) k_emit(const AxgParams p, int do
 
 int axg_diffuse_tile() { return DIFF_TILE; }
 
-void axg_launch_diffuse(const AxgParams& p, int grid, cudaStream_t s) { k_diffuse<<<grid, DIFF_THREADS, 0, s>>>(p); }
+void axg_launch_diffuse(const AxgParams& p, int grid, cudaStream_t s) {
+    if (p.bin_mode == AXG_BIN_COUNT_D) k_diffuse_chunked<<<grid, DIFF_THREADS, 0, s>>>(p);
+    else k_diffuse<<<grid, DIFF_THREADS, 0, s>>>(p);
+}
 void axg_launch_rekey(const AxgParams& p, int grid, cudaStream_t s) { k_rekey<<<grid, 256, 0, s>>>(p); }
 void axg_launch_emit(const AxgParams& p, int do_emit, cudaStream_t s) { k_emit<<<1, EMIT_THREADS, 0, s>>>(p, do_emit); }
