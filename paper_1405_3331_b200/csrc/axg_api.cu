@@ -200,8 +200,9 @@ int alloc_particles(axg_ctx* c, uint64_t cap, AxgParams& P, std::vector<void*>& 
                             n * 16, n,                      // Brec, Bsp
                             n * 4, n * 4, n * 4, n * 4, n * 4,  // key_pre, skey[2], sidx[2]
                             diff_tiles * 8, sort_tiles * AXG_RADIX * 8,
-                            (n / AXG_CHUNK + 4) * 4, (n / AXG_CHUNK + 4) * 4};  // chunk_cnt, chunk_base
-    constexpr int NB = 16;
+                            (n / AXG_CHUNK + 4) * 4, (n / AXG_CHUNK + 4) * 4,   // chunk_cnt, chunk_base
+                            n * 4, AXG_MAX_SOURCES * 4};                        // arr_pre, src_arr
+    constexpr int NB = 18;
     void* ptr[NB];
     for (int i = 0; i < NB; ++i) {
         ptr[i] = dev_alloc(c, sizes[i]);
@@ -222,6 +223,8 @@ int alloc_particles(axg_ctx* c, uint64_t cap, AxgParams& P, std::vector<void*>& 
     P.sort_state = (unsigned long long*)ptr[13];
     P.chunk_cnt = (uint32_t*)ptr[14];
     P.chunk_base = (uint32_t*)ptr[15];
+    P.arr_pre = (uint32_t*)ptr[16];
+    P.src_arr = (uint32_t*)ptr[17];
     P.capacity = (uint32_t)cap;
     // look-back words must not alias a live epoch: zero them (epoch 0 words with flag 0 = not ready)
     CU(c, cudaMemsetAsync(ptr[12], 0, sizes[12], c->stream));

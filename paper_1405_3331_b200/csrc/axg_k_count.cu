@@ -7,8 +7,8 @@
 // and P2 is
 //   k_cell_scan  cell_lo = exclusive scan of cnt over the cells (single pass, decoupled look-back)  -> O6 for free;
 //                cnt is re-zeroed on the way
-//   k_place      slot[atomicAdd(cursor of the cell)] = pre-sort index (| species << 30): cells are contiguous, the
-//                order INSIDE a cell is the arbitrary order of the atomics
+//   k_place      slot[cell_lo[key] + arrival rank] = pre-sort row (| species << 30): cells are contiguous, the order
+//                INSIDE a cell is the arbitrary order in which P1's counting atomics arrived (they return the rank)
 //   k_settle     every slot finds its rank among the members of its cell by pre-sort index (the order std::stable_sort
 //                gives equal keys, reading A-9), and the record moves to cell_lo + rank: O4 + O5.  Deterministic:
 //                nothing of the arrival order survives.
@@ -81,10 +81,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_cell_scan(const AxgParams p) {
             if (lane == 0) s_base = excl;
         }
         __syncthreads();
-        // cnt is counted SHIFTED by one cell (P1 adds to cnt[key + 1]), so this plain exclusive scan leaves in
-        // cell_lo[j] the particles below cell j - 1 = the cursor of cell j - 1.  k_place bumps cell_lo[key + 1] once per
-        // particle of cell `key`, which turns the entry into the particles below cell key + 1: after k_place the array
-        // is the exclusive scan of the true counts, with no second array and no gather.  cnt is re-zeroed on the way.
+        // cell_lo[j] = particles below cell j = where cell j starts; cell_lo[cells] = n_live.  cnt is re-zeroed on the way.
         const uint32_t wbase = s_base + woff;
         const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
 #pragma unroll
@@ -106,28 +103,23 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_cell_scan(const AxgParams p) {
     }
 }
 
-// ---- slot[cursor(key)++] = pre-sort index | species << 30 ---------------------------------------------------------
+// ---- slot[cell start + arrival rank] = pre-sort row | species << 30 ---------------------------------------------------------
 constexpr int PLACE_THREADS = 256;
-
-// the cursor of cell k lives in cell_lo[k + 1] (see k_cell_scan): one L2 atomic, no other access to the cell arrays
-__device__ __forceinline__ uint32_t take_slot(uint32_t* __restrict__ cell_lo, uint32_t k) {
-    return atomicAdd(cell_lo + k + 1u, 1u);
-}
 
 __global__ void __launch_bounds__(PLACE_THREADS) k_place(const AxgParams p) {
     // B is in the chunked layout of k_diffuse_chunked: every physical row below n_pp is visited, the holes at the end
     // of each chunk are skipped, and the slot value is the PHYSICAL row (it orders the rows like the dense index)
     const uint32_t n_phys = p.dev->n_phys, n_pp = p.dev->n_pp;
     uint32_t* __restrict__ slot = p.sidx[p.final_buf ^ 1];
-    uint32_t* __restrict__ cell_lo = p.cell_lo;
-    // one particle per thread: measured faster than four per thread with 128-bit loads (0.176 vs 0.213 ms at C3) -- the
-    // kernel is bound by L2 transactions (one atomic + one scattered 4-byte store each) and wants many warps in flight
+    const uint32_t* __restrict__ cell_lo = p.cell_lo;
+    // one particle per thread: the kernel is bound by L2 transactions (one random 4-byte read of the cell start + one
+    // scattered 4-byte store each) and wants many warps in flight.  No atomic: the counting atomic of P1 already
+    // returned every row's arrival rank inside its cell (arr_pre), in the arbitrary order of the atomics.
     for (uint32_t o = blockIdx.x * PLACE_THREADS + threadIdx.x; o < n_pp; o += gridDim.x * PLACE_THREADS) {
         if (o < n_phys && (o % AXG_CHUNK) >= __ldg(p.chunk_cnt + o / AXG_CHUNK)) continue;  // a hole
         const uint32_t k = __ldg(p.key_pre + o);
         const uint32_t sp = __ldg(p.Bsp + o);
-        // bumping the cursor hands out the slots of the cell in the arbitrary order of the atomics
-        slot[take_slot(cell_lo, k)] = o | (sp << 30);
+        slot[__ldg(cell_lo + k) + __ldg(p.arr_pre + o)] = o | (sp << 30);
     }
 }
 

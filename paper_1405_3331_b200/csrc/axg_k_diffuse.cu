@@ -18,9 +18,9 @@ constexpr int DIFF_WARPS = DIFF_THREADS / 32;
 
 // What P1 leaves for P2 besides the key: radix mode -- the digit histograms of every pass (shared memory, flushed
 // once per block); count mode -- one more particle in cnt[key] (L2 reduction, no return value).
-__device__ __forceinline__ void tally(const AxgParams& p, uint32_t (*s_hist)[AXG_RADIX], uint32_t key) {
+__device__ __forceinline__ void tally(const AxgParams& p, uint32_t (*s_hist)[AXG_RADIX], uint32_t key, uint32_t o) {
     if (p.bin_mode == AXG_BIN_COUNT_D) {
-        atomicAdd(p.cnt + key + 1u, 1u);  // shifted by one cell (see k_cell_scan); result unused: a fire-and-forget RED
+        p.arr_pre[o] = atomicAdd(p.cnt + key, 1u);  // the old count = this row's arrival rank inside its cell
     } else {
 #pragma unroll
         for (int q = 0; q < AXG_MAX_PASSES; ++q)
@@ -64,13 +64,23 @@ __device__ void emit_and_close(const AxgParams& p, int do_emit, uint32_t (*s_his
             p.Bsp[o] = (uint8_t)(sd.species_polarity & 0xffu);
             p.key_pre[o] = key;
             if (p.bin_mode != AXG_BIN_COUNT_D) {
-                tally(p, s_hist, key);
-            } else if (j == 0u) {  // all newborns of a source share its cell: one reduction per source, not per particle
-                atomicAdd(p.cnt + key + 1u, p.src_emit_prefix[s + 1] - p.src_emit_prefix[s]);
+                tally(p, s_hist, key, o);
+            } else if (j == 0u) {  // all newborns of a source share its cell: one atomic per source, not per particle
+                p.src_arr[s] = atomicAdd(p.cnt + key, p.src_emit_prefix[s + 1] - p.src_emit_prefix[s]);
             }
         }
     }
     __syncthreads();
+    if (do_emit && fits && p.bin_mode == AXG_BIN_COUNT_D) {  // arrival ranks of the newborns: source base + j
+        for (uint32_t e = tid; e < p.e_owned; e += nthr) {
+            uint32_t lo = 0u, hi = p.n_src;
+            while (hi - lo > 1u) {
+                const uint32_t mid = (lo + hi) >> 1;
+                if (p.src_emit_prefix[mid] <= e) lo = mid; else hi = mid;
+            }
+            p.arr_pre[n_phys + e] = p.src_arr[lo] + (e - p.src_emit_prefix[lo]);
+        }
+    }
     if (p.bin_mode != AXG_BIN_COUNT_D) {
         // total histogram -> exclusive scan per pass; needs >= 256 threads (one digit each)
         for (int q = 0; q < p.n_pass; ++q) {
@@ -233,7 +243,7 @@ __global__ void __launch_bounds__(DIFF_THREADS, 4) k_diffuse(const AxgParams p) 
                 s_rec[o] = make_float4(x[i], y[i], z[i], __uint_as_float(id[i]));
                 s_sp[o] = (uint8_t)((sp_pack[i >> 2] >> (8 * (i & 3))) & 0xffu);
                 s_key[o] = key;
-                tally(p, s_hist, key);
+                tally(p, s_hist, key, 0u);  // radix binning only: count binning runs k_diffuse_chunked
             }
             out += __popc(b);
         }
@@ -292,28 +302,43 @@ __global__ void __launch_bounds__(DIFF_THREADS, 4) k_diffuse_chunked(const AxgPa
         for (int i = 0; i < DIFF_ITEMS; ++i) {
             const uint32_t g = first + i * 32;
             const bool v = g < n_in;
-            x[i] = v ? __ldg(p.A.x + g) : -1.0f;
-            y[i] = v ? __ldg(p.A.y + g) : -1.0f;
-            z[i] = v ? __ldg(p.A.z + g) : -1.0f;
-            id[i] = v ? __ldg(p.A.id + g) : 0u;
-            sp[i] = v ? (uint32_t)__ldg(p.A.species + g) : 0u;
+            // volatile asm: all twenty loads of the chunk are ISSUED here, before the arithmetic of its first row (left
+            // to itself the compiler sinks each row's loads to their use, behind the previous row's divergent stores,
+            // and every row then pays a full memory latency: 42 % of the stall samples)
+            x[i] = -1.0f; y[i] = -1.0f; z[i] = -1.0f; id[i] = 0u; sp[i] = 0u;
+            if (v) {
+                asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(x[i]) : "l"(p.A.x + g) : "memory");
+                asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(y[i]) : "l"(p.A.y + g) : "memory");
+                asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(z[i]) : "l"(p.A.z + g) : "memory");
+                asm volatile("ld.global.nc.u32 %0, [%1];" : "=r"(id[i]) : "l"(p.A.id + g) : "memory");
+                asm volatile("ld.global.nc.u8 %0, [%1];" : "=r"(sp[i]) : "l"(p.A.species + g) : "memory");
+            }
+        }
+        // O1 + P1b for the four rows first, as straight-line code (the compiler interleaves the four Philox chains);
+        // the divergent part -- ranks and stores -- comes after
+        uint32_t alive = 0u;
+#pragma unroll
+        for (int i = 0; i < DIFF_ITEMS; ++i) {
+            float z0, z1, z2;
+            axg_normals3(id[i], t, 0u, rk, z0, z1, z2);
+            x[i] = fmaf(p.sigma, z0, x[i]);
+            y[i] = fmaf(p.sigma, z1, y[i]);
+            z[i] = fmaf(p.sigma, z2, z[i]);
+            const bool in = x[i] >= 0.0f && x[i] < p.fnx && y[i] >= 0.0f && y[i] < p.fny && z[i] >= 0.0f && z[i] < p.fnz;
+            alive |= ((first + i * 32) < n_in && in) ? (1u << i) : 0u;
         }
         uint32_t out = chunk * AXG_CHUNK;
 #pragma unroll
-        for (int i = 0; i < DIFF_ITEMS; ++i) {
-            const bool v = (first + i * 32) < n_in;
-            float z0, z1, z2;
-            axg_normals3(id[i], t, 0u, rk, z0, z1, z2);                       // O1
-            const float xn = fmaf(p.sigma, z0, x[i]), yn = fmaf(p.sigma, z1, y[i]), zn = fmaf(p.sigma, z2, z[i]);
-            const bool in = xn >= 0.0f && xn < p.fnx && yn >= 0.0f && yn < p.fny && zn >= 0.0f && zn < p.fnz;  // P1b
-            const uint32_t b = __ballot_sync(0xffffffffu, v && in);
-            if (v && in) {                                                     // P1d + P2a
+        for (int i = 0; i < DIFF_ITEMS; ++i) {  // P1d + P2a
+            const bool a = (alive >> i) & 1u;
+            const uint32_t b = __ballot_sync(0xffffffffu, a);
+            if (a) {
                 const uint32_t o = out + __popc(b & lt);
-                const uint32_t key = axg_cell_key(p, xn, yn, zn);
-                p.Brec[o] = make_float4(xn, yn, zn, __uint_as_float(id[i]));
+                const uint32_t key = axg_cell_key(p, x[i], y[i], z[i]);
+                p.Brec[o] = make_float4(x[i], y[i], z[i], __uint_as_float(id[i]));
                 p.Bsp[o] = (uint8_t)sp[i];
                 p.key_pre[o] = key;
-                atomicAdd(p.cnt + key + 1u, 1u);  // fire-and-forget RED (see tally)
+                p.arr_pre[o] = atomicAdd(p.cnt + key, 1u);  // old count = arrival rank inside the cell (see tally)
             }
             out += __popc(b);
         }
@@ -347,7 +372,7 @@ __global__ void __launch_bounds__(256) k_rekey(const AxgParams p) {
         p.Bsp[g] = p.A.species[g];
         p.key_pre[g] = key;
         if (p.bin_mode == AXG_BIN_COUNT_D && (g % AXG_CHUNK) == 0u) p.chunk_cnt[g / AXG_CHUNK] = min(AXG_CHUNK, n - g);
-        tally(p, s_hist, key);
+        tally(p, s_hist, key, g);
     }
     __syncthreads();
     for (int i = threadIdx.x; i < p.n_pass * AXG_RADIX; i += blockDim.x) {
