@@ -328,20 +328,24 @@ __global__ void __launch_bounds__(DIFF_THREADS, 4) k_diffuse_chunked(const AxgPa
             alive |= ((first + i * 32) < n_in && in) ? (1u << i) : 0u;
         }
         uint32_t out = chunk * AXG_CHUNK;
+        uint32_t dst[DIFF_ITEMS], arr[DIFF_ITEMS];
 #pragma unroll
         for (int i = 0; i < DIFF_ITEMS; ++i) {  // P1d + P2a
             const bool a = (alive >> i) & 1u;
             const uint32_t b = __ballot_sync(0xffffffffu, a);
+            dst[i] = out + __popc(b & lt);
             if (a) {
-                const uint32_t o = out + __popc(b & lt);
                 const uint32_t key = axg_cell_key(p, x[i], y[i], z[i]);
-                p.Brec[o] = make_float4(x[i], y[i], z[i], __uint_as_float(id[i]));
-                p.Bsp[o] = (uint8_t)sp[i];
-                p.key_pre[o] = key;
-                p.arr_pre[o] = atomicAdd(p.cnt + key, 1u);  // old count = arrival rank inside the cell (see tally)
+                arr[i] = atomicAdd(p.cnt + key, 1u);  // old count = arrival rank inside the cell (see tally)
+                p.Brec[dst[i]] = make_float4(x[i], y[i], z[i], __uint_as_float(id[i]));
+                p.Bsp[dst[i]] = (uint8_t)sp[i];
+                p.key_pre[dst[i]] = key;
             }
             out += __popc(b);
         }
+#pragma unroll
+        for (int i = 0; i < DIFF_ITEMS; ++i)  // the four atomics have been in flight together: one wait, not four
+            if ((alive >> i) & 1u) p.arr_pre[dst[i]] = arr[i];  // (storing them a trip later gains nothing: measured)
         if (lane == 0) {
             const uint32_t c = out - chunk * AXG_CHUNK;
             p.chunk_cnt[chunk] = c;
