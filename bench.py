@@ -80,9 +80,9 @@ def bytes_model(w, n_live, n_active_cones, n_stencil, count_mode):
     sense = float(per_cone) * n_active_cones
     step = (38.0 + 12.0 + 16.0 * (passes - 1) + 42.0) * n_live + 8.0 * w.cells + sense
     if count_mode:
-        k = {"diffuse": (38.0 + 4.0) * n_live,    # + the 4 B reduction on cnt[key + 1]
+        k = {"diffuse": (38.0 + 8.0) * n_live,    # + the 4 B counting atomic on cnt[key] and the 4 B arrival rank it returns
              "scan": 12.0 * (w.cells + 1),         # read cnt, write cell_lo, re-zero cnt
-             "place": 17.0 * n_live,               # key 4 + species 1 + cursor read-modify-write 8 + slot 4
+             "place": 17.0 * n_live,               # key 4 + species 1 + arrival rank 4 + cell start 4 + slot 4
              "settle": 53.0 * n_live,              # slot 4 + record 16 + cell_lo 8 + SoA 17 + key 4 + perm 4
              "sense": sense}
         launches = {"diffuse": 1, "scan": 1, "place": 1, "settle": 1, "sense": 1}
@@ -317,7 +317,7 @@ def run_ours(args, w):
     if ktimes is not None:
         step_bytes, bm, launches_of = bytes_model(w, n_avg, active, n_stencil, count_mode)
         per_step_ms = {k: v / K for k, v in ktimes.items()}
-        kernel_name = {"diffuse": "k_diffuse", "sort": "k_sort_pass", "reorder": "k_reorder", "sense": "k_sense",
+        kernel_name = {"diffuse": "k_diffuse_chunked" if count_mode else "k_diffuse", "sort": "k_sort_pass", "reorder": "k_reorder", "sense": "k_sense",
                        "scan": "k_cell_scan", "place": "k_place", "settle": "k_settle"}
         dom = max(bm.keys(), key=lambda k: per_step_ms[k])
         per_launch_ms = per_step_ms[dom] / launches_of[dom]

@@ -169,14 +169,15 @@ int axg_set_shard(axg_ctx* ctx, uint32_t rank, uint32_t world);
 /* How P2 (binning) is computed; the results are identical bit for bit.
  *  AXG_BIN_RADIX  stable LSD radix sort of (key, index), 8-bit digits, one onesweep pass per digit, then the
  *                 reorder + cell-range kernel.  Cost ~ passes x N; independent of the number of cells.
- *  AXG_BIN_COUNT  counting sort over the cells: P1 counts particles per cell (one L2 atomic each), a single-pass
- *                 scan over the cells gives the cell ranges, and a rank-inside-the-cell kernel restores the stable
- *                 order.  Cost ~ N + cells; 4 B x cells of extra device memory.
- *  AXG_BIN_AUTO   (default) COUNT when cells <= AXG_AUTO_COUNT_MAX_CELLS (the count array fits the L2 cache) and
- *                 cells <= 4 x particle capacity, else RADIX.
+ *  AXG_BIN_COUNT  counting sort over the cells: P1 counts particles per cell (one atomic each, which also returns the
+ *                 particle's arrival rank inside its cell), a single-pass scan over the cells gives the cell ranges,
+ *                 and a rank-inside-the-cell kernel restores the stable order.  Cost ~ N + cells; 4 B x cells of
+ *                 extra device memory.  Measured faster than RADIX on every config of BASELINE.json.
+ *  AXG_BIN_AUTO   (default) COUNT when cells <= 4 x particle capacity (a sparse population in a huge grid pays
+ *                 per cell) and cells <= AXG_AUTO_COUNT_MAX_CELLS, else RADIX.
  * Allowed whenever no step is half done (not between AXG_PHASE_DIFFUSE and AXG_PHASE_BIN): AXG_ESTATE.    */
 enum { AXG_BIN_AUTO = 0, AXG_BIN_RADIX = 1, AXG_BIN_COUNT = 2 };
-#define AXG_AUTO_COUNT_MAX_CELLS 20000000u
+#define AXG_AUTO_COUNT_MAX_CELLS 2147483648u
 int axg_set_binning(axg_ctx* ctx, int mode);
 
 /* Device pointer (int32[C][AXG_MAX_SPECIES][4] = n,Mx,My,Mz) of the per-cone sensing sums, for the NCCL

@@ -28,7 +28,7 @@ PHASE_DIFFUSE, PHASE_BIN, PHASE_SENSE, PHASE_ADVANCE, PHASE_COMMIT, PHASE_ALL = 
 COUNTER_NAMES = ("step", "n_live", "next_id", "emitted", "absorbed", "active", "arrived", "exited")
 KERNEL_NAMES = ("clear", "diffuse", "emit", "sort", "reorder", "sense", "advance", "commit", "scan", "place", "settle")
 BIN_AUTO, BIN_RADIX, BIN_COUNT = 0, 1, 2
-AUTO_COUNT_MAX_CELLS = 20_000_000   # include/axg.h AXG_AUTO_COUNT_MAX_CELLS
+AUTO_COUNT_MAX_CELLS = 1 << 31   # include/axg.h AXG_AUTO_COUNT_MAX_CELLS
 EXPORTS = (
     "axg_create", "axg_place_neurons", "axg_add_source", "axg_step", "axg_read_state", "axg_destroy",
     "axg_last_error", "axg_set_capacity", "axg_load_particles", "axg_load_cones", "axg_step_phase", "axg_set_shard",

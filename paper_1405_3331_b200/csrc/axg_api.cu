@@ -235,8 +235,8 @@ int alloc_particles(axg_ctx* c, uint64_t cap, AxgParams& P, std::vector<void*>& 
 // AXG_BIN_AUTO -> a concrete mode; the count array exists (all-zero) whenever the mode is COUNT
 int resolve_binning(axg_ctx* c) {
     int mode = c->bin_request;
-    // count mode pays per cell and wants its 4 B x cells count array resident in the 126 MB L2 (measured: faster than
-    // radix at C3 = 16.8 M cells, slower at C4 = 134 M cells, where its atomics go to DRAM)
+    // count mode pays per cell (scan + 8 B x cells of memory) and per particle; measured faster than radix on C1..C5,
+    // also where the count array (C4: 0.5 GB, C5: 1 GB) is far larger than the L2
     if (mode == AXG_BIN_AUTO)
         mode = (c->cells() <= AXG_AUTO_COUNT_MAX_CELLS && c->cells() <= 4 * (size_t)c->max_particles) ? AXG_BIN_COUNT
                                                                                                       : AXG_BIN_RADIX;

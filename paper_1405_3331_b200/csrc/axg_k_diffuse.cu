@@ -279,7 +279,10 @@ __global__ void __launch_bounds__(DIFF_THREADS, 4) k_diffuse(const AxgParams p) 
 // look-back.  The position of a row in this layout orders the rows exactly as the dense index would, so the stable
 // order of P2 is unchanged; the dense index itself (the permutation the ABI reports) is chunk_base + offset, computed
 // by the export kernels only.
-__global__ void __launch_bounds__(DIFF_THREADS, 4) k_diffuse_chunked(const AxgParams p) {
+#ifndef AXG_CHUNKED_BLOCKS
+#define AXG_CHUNKED_BLOCKS 4
+#endif
+__global__ void __launch_bounds__(DIFF_THREADS, AXG_CHUNKED_BLOCKS) k_diffuse_chunked(const AxgParams p) {
     __shared__ uint32_t s_hist[AXG_MAX_PASSES][AXG_RADIX];  // scratch of emit_and_close only
     __shared__ uint32_t s_surv;
     AxgDev* dev = p.dev;
@@ -396,7 +399,7 @@ __global__ void __launch_bounds__(EMIT_THREADS) k_emit(const AxgParams p, int do
 int axg_diffuse_tile() { return DIFF_TILE; }
 
 void axg_launch_diffuse(const AxgParams& p, int grid, cudaStream_t s) {
-    if (p.bin_mode == AXG_BIN_COUNT_D) k_diffuse_chunked<<<grid, DIFF_THREADS, 0, s>>>(p);
+    if (p.bin_mode == AXG_BIN_COUNT_D) k_diffuse_chunked<<<148 * AXG_CHUNKED_BLOCKS, DIFF_THREADS, 0, s>>>(p);
     else k_diffuse<<<grid, DIFF_THREADS, 0, s>>>(p);
 }
 void axg_launch_rekey(const AxgParams& p, int grid, cudaStream_t s) { k_rekey<<<grid, 256, 0, s>>>(p); }
