@@ -42,8 +42,9 @@ NOMINAL_GBS = 8000.0          # north_star's "~8 TB/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the `ncu --set full` capture
 # summarised in profiles/ (a capture is not repeatable inside a timed run, so it is a recorded number).
 TRAFFIC_NCU = {   # (workload, kernel) -> bytes per launch; profiles/r01_summary.md
-    ("C3", "k_diffuse"): 699.7e6, ("C3", "k_settle"): 791.7e6, ("C3", "k_place"): 343.4e6, ("C3", "k_cell_scan"): 142.3e6,
-    ("C3", "k_sort_pass"): 203.2e6, ("C3", "k_reorder"): 903.4e6,
+    ("C3", "k_diffuse_chunked"): 770.1e6, ("C3", "k_diffuse"): 578.9e6, ("C3", "k_settle"): 782.1e6,
+    ("C3", "k_place"): 266.5e6, ("C3", "k_cell_scan"): 142.9e6, ("C3", "k_sort_pass"): 203.7e6,
+    ("C3", "k_reorder"): 740.8e6,
 }
 
 
