@@ -210,3 +210,15 @@ def test_binning_crowded_cells(axg, n):
     compare_binning(g, o)
     g.close()
     o.close()
+
+
+@pytest.mark.parametrize("grid", [(24, 20, 16), (6, 5, 4)])
+def test_chain_heavy_absorption(axg, grid):
+    """sigma = 4 cells on a 24 x 20 x 16 and on a 6 x 5 x 4 grid: a third to nearly all of the particles leave the box
+    in one step, so the compaction of P1 is far from the identity (count binning: chunks with few or no survivors, most
+    physical rows are holes; radix binning: long look-back sums); on the small grid the newborns are a large part of
+    what is left and every cell is crowded.  (sigma stays at 4: the position tolerance of NS is absolute, and an ulp
+    of a normal deviate times sigma must stay below it.)"""
+    w = W.small(seed=17, grid=grid, n_cones=9)
+    w.D = 8.0
+    _chain(axg, w, n=30_011, seed=19, steps=2)
