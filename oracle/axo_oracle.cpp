@@ -114,6 +114,10 @@ struct axo_ctx {
     uint64_t max_particles = 1ull << 20;
     uint32_t max_segments = 1024;
     uint32_t shard_rank = 0, shard_world = 1;
+    // steering rule of P4: 0 = vector addition (north_star), 1 = fixed turn by the sign of N(SNR, 1) (Eq. 5)
+    int steer_mode = 0;
+    float snr_gain = 1.0f, cos_turn = 1.0f, sin_turn = 0.0f;
+    uint32_t n_stencil = 0;  // |N_R|, filled by axo_set_steering
 
     std::vector<Source> sources;
     int8_t species_polarity[MAX_SPECIES] = {0, 0, 0, 0};
@@ -321,13 +325,44 @@ void phase_advance(axo_ctx* c) {
         }
         float xi[3];
         normals3(c->seed, (uint32_t)cone, t, 1u, xi, nullptr);  // stream 1 = cone noise (A-2)
-        float v[3];
-        for (int a = 0; a < 3; ++a) v[a] = g[a] + c->noise * xi[a];  // A-15
-        const float vlen = std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
-        if (vlen > 0.0f) {
-            for (int a = 0; a < 3; ++a) h[a] = v[a] / vlen;
+        if (c->steer_mode == 1) {
+            // The paper's first steering rule (Eq. 5; reading A-25): a turn of fixed size delta
+            // towards ("right") or away from ("left") the gradient direction, by the sign of a draw from N(SNR, 1),
+            //   SNR = gain * mu * sqrt(gamma / (1 + gamma)^3) * sin(phi),
+            // gamma = particles per cell in range (background concentration), mu = |g| / gamma (relative gradient per
+            // cell, g = G / S2), phi = angle between the heading and the gradient direction.  In 3-D the turn is the
+            // rotation of the heading by delta in the plane spanned by heading and gradient.  Nothing in range, G = 0
+            // or heading parallel to the gradient: keep the direction.
+            int64_t n_all = 0;
+            for (int s = 0; s < MAX_SPECIES; ++s) n_all += c->cone_counts[cone * MAX_SPECIES + s];
+            const float dot = h[0] * g[0] + h[1] * g[1] + h[2] * g[2];
+            float w[3];
+            for (int a = 0; a < 3; ++a) w[a] = g[a] - dot * h[a];  // part of the gradient direction orthogonal to h
+            const float sinphi = std::sqrt(w[0] * w[0] + w[1] * w[1] + w[2] * w[2]);
+            const bool have_g = !(G[0] == 0 && G[1] == 0 && G[2] == 0);
+            if (have_g && n_all > 0 && sinphi > 0.0f) {
+                const float gx = (float)G[0], gy = (float)G[1], gz = (float)G[2];
+                const float glen = std::sqrt(gx * gx + gy * gy + gz * gz) / (float)stencil_S2(
+                                       (int)std::floor((double)c->radius * (double)c->radius));
+                const float gamma = (float)n_all / (float)c->n_stencil;
+                const float mu = glen / gamma;
+                const float one = 1.0f + gamma;
+                const float snr = c->snr_gain * mu * std::sqrt(gamma / (one * one * one)) * sinphi;
+                const float sgn = (snr + xi[0] > 0.0f) ? 1.0f : -1.0f;
+                float v[3];
+                for (int a = 0; a < 3; ++a) v[a] = c->cos_turn * h[a] + (sgn * c->sin_turn) * (w[a] / sinphi);
+                const float vlen = std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+                for (int a = 0; a < 3; ++a) h[a] = v[a] / vlen;
+            }
         } else {
-            for (int a = 0; a < 3; ++a) h[a] = g[a];
+            float v[3];
+            for (int a = 0; a < 3; ++a) v[a] = g[a] + c->noise * xi[a];  // A-15
+            const float vlen = std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+            if (vlen > 0.0f) {
+                for (int a = 0; a < 3; ++a) h[a] = v[a] / vlen;
+            } else {
+                for (int a = 0; a < 3; ++a) h[a] = g[a];
+            }
         }
         for (int a = 0; a < 3; ++a) p[a] = p[a] + c->speed * h[a];  // P:282 fixed distance per step
         // O9 append (a capsule is added at the end of the previous one)
@@ -476,6 +511,25 @@ AXO_API int axo_add_source(axo_ctx* c, float x, float y, float z, uint8_t specie
 AXO_API int axo_set_shard(axo_ctx* c, uint32_t rank, uint32_t world) {
     if (!c || world == 0 || rank >= world) return fail(c, EINVAL_, "bad shard");
     c->shard_rank = rank; c->shard_world = world;
+    return OK;
+}
+
+// mode 0 = vector addition (default), 1 = fixed turn by the sign of N(SNR, 1); gain >= 0; 0 < turn < pi (radians)
+AXO_API int axo_set_steering(axo_ctx* c, int mode, float gain, float turn) {
+    if (!c || (mode != 0 && mode != 1) || !(gain >= 0.0f) || !std::isfinite(gain) || !(turn > 0.0f) ||
+        !(turn < 3.14159265f))
+        return fail(c, EINVAL_, "bad steering mode / gain / turn");
+    c->steer_mode = mode;
+    c->snr_gain = gain;
+    c->cos_turn = (float)std::cos((double)turn);
+    c->sin_turn = (float)std::sin((double)turn);
+    const int r2 = (int)std::floor((double)c->radius * (double)c->radius), R = (int)std::floor((double)c->radius);
+    uint32_t cells = 0;
+    for (int dz = -R; dz <= R; ++dz)
+        for (int dy = -R; dy <= R; ++dy)
+            for (int dx = -R; dx <= R; ++dx)
+                if (dx * dx + dy * dy + dz * dz <= r2) ++cells;
+    c->n_stencil = cells;
     return OK;
 }
 
