@@ -180,6 +180,19 @@ enum { AXG_BIN_AUTO = 0, AXG_BIN_RADIX = 1, AXG_BIN_COUNT = 2 };
 #define AXG_AUTO_COUNT_MAX_CELLS 2147483648u
 int axg_set_binning(axg_ctx* ctx, int mode);
 
+/* Steering rule of P4.
+ *  AXG_STEER_VECTOR (default)  north_star's rule: heading = normalise(gradient direction + noise x N(0, I)).
+ *  AXG_STEER_SNR    the paper's first rule (Eq. 5; reading A-25): the heading turns by the
+ *                   fixed angle `turn` (radians; the paper's pi/30) in the plane of heading and gradient, TOWARDS the
+ *                   gradient direction if a draw from N(SNR, 1) is positive, away from it otherwise, with
+ *                   SNR = gain x mu x sqrt(gamma / (1 + gamma)^3) x sin(phi); gamma = particles per cell over the
+ *                   sensing stencil, mu = |g| / gamma (g = the gradient estimate of P3), phi = angle between heading
+ *                   and gradient.  Nothing in range, zero gradient or heading parallel to it: direction kept.  The
+ *                   draw is the first normal of the cone's Philox block (stream 1); `noise` is not used.
+ * gain >= 0, 0 < turn < pi, else AXG_EINVAL.  May be called between any two steps.                         */
+enum { AXG_STEER_VECTOR = 0, AXG_STEER_SNR = 1 };
+int axg_set_steering(axg_ctx* ctx, int mode, float gain, float turn);
+
 /* Device pointer (int32[C][AXG_MAX_SPECIES][4] = n,Mx,My,Mz) of the per-cone sensing sums, for the NCCL
  * all-reduce between P3 and P4 when sharded.  *bytes = its size.  Owned by ctx.                           */
 int axg_sense_buffer(axg_ctx* ctx, void** device_ptr, size_t* bytes);

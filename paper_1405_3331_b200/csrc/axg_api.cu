@@ -545,6 +545,17 @@ AXG_API int axg_set_binning(axg_ctx* c, int mode) {
     return c->particles_allocated ? resolve_binning(c) : AXG_OK;
 }
 
+AXG_API int axg_set_steering(axg_ctx* c, int mode, float gain, float turn) {
+    if (!c || (mode != AXG_STEER_VECTOR && mode != AXG_STEER_SNR) || !(gain >= 0.0f) || !std::isfinite(gain) ||
+        !(turn > 0.0f) || !(turn < 3.14159265f))
+        return fail(c, AXG_EINVAL, "bad steering mode / gain / turn");
+    c->P.steer_mode = mode;
+    c->P.snr_gain = gain;
+    c->P.cos_turn = (float)std::cos((double)turn);
+    c->P.sin_turn = (float)std::sin((double)turn);
+    return AXG_OK;
+}
+
 AXG_API int axg_add_source(axg_ctx* c, float x, float y, float z, uint8_t species, int8_t polarity, uint32_t rate) {
     if (!c) return AXG_EINVAL;
     if (!inside(c, x, y, z)) return fail(c, AXG_EINVAL, "source outside the domain");

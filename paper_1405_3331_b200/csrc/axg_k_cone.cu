@@ -73,10 +73,11 @@ __global__ void __launch_bounds__(128) k_advance(const AxgParams p, int commit) 
     const AxgRoundKeys rk = axg_round_keys(p.seed_lo, p.seed_hi);
     for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < p.n_cones; c += gridDim.x * blockDim.x) {
         if (p.cone_state[c] != 0) continue;
-        long long G[3] = {0, 0, 0};
+        long long G[3] = {0, 0, 0}, n_all = 0;
 #pragma unroll
         for (int s = 0; s < AXG_MAX_SPECIES_D; ++s) {
             const int4 v = *reinterpret_cast<const int4*>(p.sense + (size_t)c * 16 + s * 4);
+            n_all += v.x;
             G[0] += (long long)p.polarity[s] * v.y;
             G[1] += (long long)p.polarity[s] * v.z;
             G[2] += (long long)p.polarity[s] * v.w;
@@ -96,13 +97,44 @@ __global__ void __launch_bounds__(128) k_advance(const AxgParams p, int commit) 
         }
         float xi[3];
         axg_normals3(c, t, 1u, rk, xi[0], xi[1], xi[2]);  // stream 1 = cone noise (A-2)
-        float v[3];
+        if (p.steer_mode == 1) {
+            // the paper's first steering rule (Eq. 5; reading A-25): fixed turn towards / away from the
+            // gradient direction by the sign of a draw from N(SNR, 1).  Same operations, in the same order, as the oracle.
+            const float dot = __fadd_rn(__fadd_rn(__fmul_rn(h[0], g[0]), __fmul_rn(h[1], g[1])), __fmul_rn(h[2], g[2]));
+            float w[3];
 #pragma unroll
-        for (int a = 0; a < 3; ++a) v[a] = __fadd_rn(g[a], __fmul_rn(p.noise, xi[a]));  // reading A-15
-        const float vlen =
-            __fsqrt_rn(__fadd_rn(__fadd_rn(__fmul_rn(v[0], v[0]), __fmul_rn(v[1], v[1])), __fmul_rn(v[2], v[2])));
+            for (int a = 0; a < 3; ++a) w[a] = __fsub_rn(g[a], __fmul_rn(dot, h[a]));
+            const float sinphi =
+                __fsqrt_rn(__fadd_rn(__fadd_rn(__fmul_rn(w[0], w[0]), __fmul_rn(w[1], w[1])), __fmul_rn(w[2], w[2])));
+            const bool have_g = !(G[0] == 0 && G[1] == 0 && G[2] == 0);
+            if (have_g && n_all > 0 && sinphi > 0.0f) {
+                const float glen = __fdiv_rn(
+                    __fsqrt_rn(__fadd_rn(__fadd_rn(__fmul_rn(gx, gx), __fmul_rn(gy, gy)), __fmul_rn(gz, gz))), p.s2);
+                const float gamma = __fdiv_rn((float)n_all, (float)p.n_stencil);
+                const float mu = __fdiv_rn(glen, gamma);
+                const float one = __fadd_rn(1.0f, gamma);
+                const float root = __fsqrt_rn(__fdiv_rn(gamma, __fmul_rn(__fmul_rn(one, one), one)));
+                const float snr = __fmul_rn(__fmul_rn(__fmul_rn(p.snr_gain, mu), root), sinphi);
+                const float sgn = (__fadd_rn(snr, xi[0]) > 0.0f) ? 1.0f : -1.0f;
+                const float st = __fmul_rn(sgn, p.sin_turn);
+                float v[3];
 #pragma unroll
-        for (int a = 0; a < 3; ++a) h[a] = (vlen > 0.0f) ? __fdiv_rn(v[a], vlen) : g[a];
+                for (int a = 0; a < 3; ++a)
+                    v[a] = __fadd_rn(__fmul_rn(p.cos_turn, h[a]), __fmul_rn(st, __fdiv_rn(w[a], sinphi)));
+                const float vlen =
+                    __fsqrt_rn(__fadd_rn(__fadd_rn(__fmul_rn(v[0], v[0]), __fmul_rn(v[1], v[1])), __fmul_rn(v[2], v[2])));
+#pragma unroll
+                for (int a = 0; a < 3; ++a) h[a] = __fdiv_rn(v[a], vlen);
+            }
+        } else {
+            float v[3];
+#pragma unroll
+            for (int a = 0; a < 3; ++a) v[a] = __fadd_rn(g[a], __fmul_rn(p.noise, xi[a]));  // reading A-15
+            const float vlen =
+                __fsqrt_rn(__fadd_rn(__fadd_rn(__fmul_rn(v[0], v[0]), __fmul_rn(v[1], v[1])), __fmul_rn(v[2], v[2])));
+#pragma unroll
+            for (int a = 0; a < 3; ++a) h[a] = (vlen > 0.0f) ? __fdiv_rn(v[a], vlen) : g[a];
+        }
 #pragma unroll
         for (int a = 0; a < 3; ++a) q[a] = __fadd_rn(q[a], __fmul_rn(p.speed, h[a]));
 #pragma unroll

@@ -27,10 +27,13 @@ def axg(request):
     pu.BINNING = None
 
 
-def _chain(axg, w, n, seed, steps=2, n_species=2):
+def _chain(axg, w, n, seed, steps=2, n_species=2, steering=None):
     """load -> [P1 | P2 | P3 | P4+P5] x steps, each phase compared; the oracle is re-fed the GPU's P1 output so that
     integer phases are compared on identical inputs."""
     g, o = make_pair(w, axg)
+    if steering is not None:
+        g.set_steering(*steering)
+        o.set_steering(*steering)
     load_same_particles(g, o, seed, n, w.grid, n_species=n_species, step=3)
     flips = 0
     for k in range(steps):
@@ -222,3 +225,13 @@ def test_chain_heavy_absorption(axg, grid):
     w = W.small(seed=17, grid=grid, n_cones=9)
     w.D = 8.0
     _chain(axg, w, n=30_011, seed=19, steps=2)
+
+
+def test_chain_snr_steering(axg):
+    """the paper's first steering rule (fixed turn pi/30 by the sign of N(SNR, 1), Eq. 5) on both
+    sides; the decision is taken in fp32 with the same operations in the same order, so headings agree within NS's
+    tolerance unless SNR + xi is within an ulp of zero.  Gains chosen so that turns towards and away both occur."""
+    import math
+    for gain in (0.0, 8.0):
+        w = W.small(seed=23, n_cones=400, grid=(24, 20, 16))
+        _chain(axg, w, n=60_013, seed=29, steps=3, steering=(1, gain, math.pi / 30))
