@@ -72,3 +72,60 @@ def test_count_binning_equals_radix_binning(axg):
 def test_count_equals_radix_with_the_fixed_turn_rule(axg):
     st = (1, 8.0, np.pi / 30)
     _same(_run(axg, axg.BIN_COUNT, [STEPS], st), _run(axg, axg.BIN_RADIX, [STEPS], st))
+
+
+def test_two_shards_on_one_gpu_equal_the_unsharded_run(axg):
+    """DESIGN.md §8 on the real library: two contexts sharded by source (axg_set_shard, the enqueue / sync calls of the
+    multi-GPU loop), the all-reduce replaced by a sum of the two device buffers on the same stream.  The cones must be
+    bit-identical to the unsharded run, and the two shards' particles together must be its particles, bit for bit.
+    (One process, one GPU, the host drives both shards in turn: no kernel waits on another.)"""
+    import torch
+    from paper_1405_3331_b200 import sharded as S
+
+    steps = 40
+    w = W.small(seed=47, grid=(40, 33, 21), n_cones=200, n_sources=5, rate=150)
+    w.max_particles = 1 << 17
+
+    def make():
+        g = axg.Axg(w.grid, w.D, w.emission, w.radius, w.speed, w.noise, w.seed)
+        g.set_binning(axg.BIN_COUNT)
+        W.apply(g, w)
+        return g
+
+    ref = make()
+    ref.step(steps)
+    shards = [make() for _ in range(2)]
+    for r, g in enumerate(shards):
+        g.set_shard(r, 2)
+    bufs = []
+    for g in shards:
+        ptr, nbytes = g.sense_buffer()
+        bufs.append(torch.as_tensor(S._DevBuf(ptr, nbytes // 4), device="cuda"))
+    for g in shards:
+        g.check_capacity(steps)
+    for _ in range(steps):
+        for g in shards:
+            g.enqueue_phase(S.PHASE_DIFFUSE | S.PHASE_BIN | S.PHASE_SENSE)
+        total = bufs[0] + bufs[1]          # torch's current stream = the stream of both contexts
+        bufs[0].copy_(total)
+        bufs[1].copy_(total)
+        for g in shards:
+            g.enqueue_phase(S.PHASE_ADVANCE | S.PHASE_COMMIT)
+    for g in shards:
+        g.sync()
+    for f in ("CONE_POS", "CONE_HEADING", "CONE_STATE", "POLY_LEN", "POLYLINE", "CONE_GRADIENT"):
+        a = ref.read_state(f)
+        for g in shards:
+            b = g.read_state(f)
+            assert np.array_equal(a.view(np.uint8), b.view(np.uint8)), f
+    cols = {k: np.concatenate([g.read_state("PART_" + k) for g in shards]) for k in ("ID", "X", "Y", "Z", "SPECIES")}
+    order, rorder = np.argsort(cols["ID"], kind="stable"), np.argsort(ref.read_state("PART_ID"), kind="stable")
+    assert len(order) == len(rorder) > 5000
+    for k in ("ID", "X", "Y", "Z", "SPECIES"):
+        a, b = ref.read_state("PART_" + k)[rorder], cols[k][order]
+        assert np.array_equal(a.view(np.uint8), b.view(np.uint8)), k
+    c = [g.counters() for g in shards]
+    assert c[0]["emitted"] + c[1]["emitted"] == ref.counters()["emitted"]
+    assert c[0]["next_id"] == c[1]["next_id"] == ref.counters()["next_id"]
+    for g in shards + [ref]:
+        g.close()
