@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -50,6 +51,14 @@ struct axg_ctx {
     cudaStream_t side = nullptr;
     cudaEvent_t ev_bin = nullptr, ev_adv = nullptr;
     bool adv_pending = false;
+    // one step of axg_step(n >= AXG_GRAPH_MIN_STEPS) as a CUDA graph (enqueue_unit), re-captured when anything it bakes in
+    // -- the parameter block, the stream -- has changed
+    cudaStream_t gstream = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    cudaGraphExec_t graph_exec = nullptr;
+    AxgParams graph_P;
+    cudaStream_t graph_stream = nullptr;
+    bool graph_cones = false;
     std::string err;
 
     // device memory
@@ -439,6 +448,108 @@ int enqueue_phases(axg_ctx* c, uint32_t mask, Prof& prof, bool overlap = false) 
     return launches;
 }
 
+// One step as axg_step(n > 1) orders it: [P3..P5 of the PREVIOUS step on the side stream || P1 of this step] -> P2 of this
+// step (which rewrites what P3 reads, hence the join before it).  Without cones: P1 -> P2 -> commit.  Everything a step
+// needs beyond the parameter block lives in device memory (AxgDev), so the unit is the same for every step and can be
+// replayed as a CUDA graph.
+int enqueue_unit(axg_ctx* c, cudaStream_t s, bool prev_cones) {
+    const AxgParams& P = c->P;
+    const bool count_mode = P.bin_mode == AXG_BIN_COUNT_D;
+    int launches = 0;
+    if (prev_cones) {
+        cudaEventRecord(c->ev_bin, s);
+        cudaStreamWaitEvent(c->side, c->ev_bin, 0);
+        axg_launch_sense(P, c->side);
+        axg_launch_advance(P, 1, c->side);  // O10 rides in its last block
+        cudaEventRecord(c->ev_adv, c->side);
+        launches += 2;
+    }
+    axg_launch_diffuse(P, N_SM * 4, s);
+    if (prev_cones) cudaStreamWaitEvent(s, c->ev_adv, 0);
+    if (count_mode) {
+        axg_launch_cell_scan(P, N_SM * 4, s);
+        axg_launch_place(P, N_SM * 8, s);
+        axg_launch_settle(P, N_SM * 8, s);
+        launches += 4;
+    } else {
+        for (int q = 0; q < P.n_pass; ++q) axg_launch_sort_pass(P, q, N_SM * 2, s);
+        axg_launch_reorder(P, N_SM * 8, c->max_particles > AXG_REORDER_WIDE_ABOVE ? 1 : 0, s);
+        launches += P.n_pass + 2;
+    }
+    if (!P.n_cones) {
+        axg_launch_commit(P, 1, s);
+        launches += 1;
+    }
+    return launches;
+}
+
+// n whole steps through the graph of one unit.  Returns the number of kernel launches, or -1 when capture failed (the
+// caller then falls back to plain enqueueing; the stream is left unharmed).
+constexpr uint32_t AXG_GRAPH_MIN_STEPS = 4;
+long long enqueue_steps_graph(axg_ctx* c, uint32_t n) {
+    const bool cones = c->P.n_cones > 0;
+    // the legacy default stream (torch's default) cannot be captured: the steps then run on a stream of the ctx's own,
+    // forked from and joined back into the caller's stream with two events
+    cudaStream_t s = c->stream;
+    const bool detour = s == nullptr || s == cudaStreamLegacy;
+    if (detour) {
+        if (!c->gstream) {
+            if (cudaStreamCreateWithFlags(&c->gstream, cudaStreamNonBlocking) != cudaSuccess ||
+                cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+                cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+                cudaGetLastError();
+                return -1;
+            }
+        }
+        s = c->gstream;
+    }
+    if (c->graph_exec && (std::memcmp(&c->graph_P, &c->P, sizeof(AxgParams)) != 0 || c->graph_stream != s ||
+                          c->graph_cones != cones)) {
+        cudaGraphExecDestroy(c->graph_exec);
+        c->graph_exec = nullptr;
+    }
+    int unit_launches = 0;
+    if (!c->graph_exec) {
+        cudaGraph_t g = nullptr;
+        if (cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return -1; }
+        unit_launches = enqueue_unit(c, s, cones);
+        if (cudaStreamEndCapture(s, &g) != cudaSuccess || !g) { cudaGetLastError(); return -1; }
+        const cudaError_t e = cudaGraphInstantiate(&c->graph_exec, g, 0);
+        cudaGraphDestroy(g);
+        if (e != cudaSuccess) { cudaGetLastError(); c->graph_exec = nullptr; return -1; }
+        std::memcpy(&c->graph_P, &c->P, sizeof(AxgParams));
+        c->graph_stream = s;
+        c->graph_cones = cones;
+    } else {
+        unit_launches = (c->P.bin_mode == AXG_BIN_COUNT_D ? 4 : c->P.n_pass + 2) + (cones ? 2 : 1);
+    }
+    if (detour) {
+        cudaEventRecord(c->ev_fork, c->stream);
+        cudaStreamWaitEvent(s, c->ev_fork, 0);
+    }
+    if (c->cnt_dirty) cudaMemsetAsync(c->d_cnt, 0, c->cells_padded() * sizeof(uint32_t), s);
+    long long launches = 0;
+    uint32_t first_graph_step = 0;
+    if (cones) {  // the first step has no previous cones to run beside its P1
+        launches += enqueue_unit(c, s, false);
+        first_graph_step = 1;
+    }
+    for (uint32_t i = first_graph_step; i < n; ++i) cudaGraphLaunch(c->graph_exec, s);
+    launches += (long long)(n - first_graph_step) * unit_launches;
+    if (cones) {  // P3..P5 of the last step
+        axg_launch_sense(c->P, s);
+        axg_launch_advance(c->P, 1, s);
+        launches += 2;
+    }
+    if (detour) {
+        cudaEventRecord(c->ev_join, s);
+        cudaStreamWaitEvent(c->stream, c->ev_join, 0);
+    }
+    c->cnt_dirty = false;
+    c->b_chunked = c->P.bin_mode == AXG_BIN_COUNT_D;
+    return launches;
+}
+
 void finish_prof(axg_ctx* c, Prof& prof) {
     if (!prof.on) return;
     for (int k = 0; k < AXG_KERNEL_COUNT; ++k) c->ktimes[k] = 0.f;
@@ -514,6 +625,10 @@ AXG_API void axg_destroy(axg_ctx* c) {
     dev_free(c->d_dev); dev_free(c->d_cell_lo); dev_free(c->d_src); dev_free(c->d_src_id_prefix);
     dev_free(c->d_src_emit_prefix); dev_free(c->d_stencil);
     for (cudaEvent_t e : c->prof_events) cudaEventDestroy(e);
+    if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    if (c->ev_join) cudaEventDestroy(c->ev_join);
+    if (c->gstream) cudaStreamDestroy(c->gstream);
     if (c->ev_bin) cudaEventDestroy(c->ev_bin);
     if (c->ev_adv) cudaEventDestroy(c->ev_adv);
     if (c->side) cudaStreamDestroy(c->side);
@@ -716,7 +831,12 @@ AXG_API int axg_step(axg_ctx* c, uint32_t n) {
         CU(c, cudaEventCreateWithFlags(&c->ev_adv, cudaEventDisableTiming));
     }
     CU(c, cudaEventRecord(c->ev0, c->stream));
-    for (uint32_t i = 0; i < n; ++i) launches += enqueue_phases(c, AXG_PHASE_ALL, prof, overlap);
+    long long graphed = -1;
+    if (!prof.on && n >= AXG_GRAPH_MIN_STEPS && (overlap || c->n_cones == 0) && !std::getenv("AXG_NO_GRAPH"))
+        graphed = enqueue_steps_graph(c, n);
+    if (graphed >= 0) launches = (uint64_t)graphed;
+    else
+        for (uint32_t i = 0; i < n; ++i) launches += enqueue_phases(c, AXG_PHASE_ALL, prof, overlap);
     if (c->adv_pending) {  // join: the ctx stream waits for the last step's cones
         CU(c, cudaStreamWaitEvent(c->stream, c->ev_adv, 0));
         c->adv_pending = false;
