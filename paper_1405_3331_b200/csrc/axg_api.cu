@@ -562,18 +562,17 @@ void finish_prof(axg_ctx* c, Prof& prof) {
 
 // host-side pre-checks from device counters: nothing is enqueued when they fail
 int capacity_check(axg_ctx* c, uint32_t n, bool diffuse, bool advance, AxgDev* h) {
+    const bool census = advance && c->n_cones;
+    if (census) {  // longest active polyline, on the stream ahead of the one read below: one synchronisation, not two
+        CU(c, cudaMemsetAsync(&((AxgDev*)c->d_dev)->cone_census[0], 0, 4 * sizeof(uint32_t), c->stream));
+        axg_launch_census(c->P, c->stream);
+    }
     int rc = read_dev(c, h);
     if (rc) return rc;
     if (diffuse && (uint64_t)h->n_live + (uint64_t)n * owned_rate(c) > c->max_particles)
         return fail(c, AXG_ECAPACITY, "particle capacity would overflow");
-    if (advance && c->n_cones) {
-        CU(c, cudaMemsetAsync(&((AxgDev*)c->d_dev)->cone_census[0], 0, 4 * sizeof(uint32_t), c->stream));
-        axg_launch_census(c->P, c->stream);
-        rc = read_dev(c, h);
-        if (rc) return rc;
-        if (h->cone_census[0] && (uint64_t)h->cone_census[3] + n > (uint64_t)c->max_segments + 1)
-            return fail(c, AXG_ECAPACITY, "polyline capacity would overflow");
-    }
+    if (census && h->cone_census[0] && (uint64_t)h->cone_census[3] + n > (uint64_t)c->max_segments + 1)
+        return fail(c, AXG_ECAPACITY, "polyline capacity would overflow");
     return AXG_OK;
 }
 
@@ -766,11 +765,17 @@ AXG_API int axg_load_particles(axg_ctx* c, const float* x, const float* y, const
                                const uint32_t* id, uint64_t n, uint32_t next_id, uint32_t step) {
     if (!c || (n && (!x || !y || !z || !species || !id))) return fail(c, AXG_EINVAL, "null argument");
     if (n > c->max_particles) return fail(c, AXG_ECAPACITY, "more particles than capacity");
-    uint32_t mask = 0;
+    // which species occur, and that none is out of range: branch-free so that the host compiler vectorises it (this loop
+    // runs over every particle of every axg_load_particles call: 16.6 M bytes at C3)
+    uint8_t any = 0, has[AXG_MAX_SPECIES] = {0, 0, 0, 0};
     for (uint64_t i = 0; i < n; ++i) {
-        if (species[i] >= AXG_MAX_SPECIES) return fail(c, AXG_EINVAL, "species >= 4");
-        mask |= 1u << species[i];
+        const uint8_t sp = species[i];
+        any |= sp;
+        has[0] |= (uint8_t)(sp == 0); has[1] |= (uint8_t)(sp == 1); has[2] |= (uint8_t)(sp == 2); has[3] |= (uint8_t)(sp == 3);
     }
+    if (any >= AXG_MAX_SPECIES) return fail(c, AXG_EINVAL, "species >= 4");
+    uint32_t mask = 0;
+    for (int sp = 0; sp < (int)AXG_MAX_SPECIES; ++sp) mask |= has[sp] ? (1u << sp) : 0u;
     int rc = ensure_particles(c);
     if (rc) return rc;
     if (n) {
@@ -844,13 +849,15 @@ AXG_API int axg_step(axg_ctx* c, uint32_t n) {
     prof.mark(-1);
     CU(c, cudaEventRecord(c->ev1, c->stream));
     c->stepped = true;
-    rc = after_sync(c, "axg_step");
+    rc = read_dev(c, &h);  // the one synchronisation of the call: the copy is queued behind the last kernel
     if (rc) return rc;
+    {
+        const cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return cuda_fail(c, e, "axg_step");
+    }
     finish_prof(c, prof);
     cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1);
     c->last_launches = launches;
-    rc = read_dev(c, &h);
-    if (rc) return rc;
     c->last_particle_steps = h.particle_steps - ps0;
     c->n_A = c->n_B = h.n_live;
     if (h.err) {
