@@ -125,7 +125,9 @@ int axg_add_source(axg_ctx* ctx, float x, float y, float z, uint8_t species, int
 /* Run n whole time steps (P1..P5 + commit each) on the device without host synchronisation in between;
  * returns after the stream has been synchronised and the device error word read.  With cones placed, P3..P5 of
  * step t run on a ctx-owned side stream concurrently with P1 of step t+1 (they share no data; joined by events
- * before P2 of step t+1 and before the call returns).                                                    */
+ * before P2 of step t+1 and before the call returns).  For n >= 4 one step is captured once as a CUDA graph and
+ * replayed (re-captured when a setting or an allocation has changed); when the ctx stream is the legacy default
+ * stream, which cannot be captured, the steps run on a ctx-owned stream forked from and joined back into it.  */
 int axg_step(axg_ctx* ctx, uint32_t n);
 
 /* Copy one field to host memory.  If dst == NULL or dst_bytes is too small: returns AXG_ESMALL (or AXG_OK when

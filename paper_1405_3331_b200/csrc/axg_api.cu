@@ -837,7 +837,7 @@ AXG_API int axg_step(axg_ctx* c, uint32_t n) {
     }
     CU(c, cudaEventRecord(c->ev0, c->stream));
     long long graphed = -1;
-    if (!prof.on && n >= AXG_GRAPH_MIN_STEPS && (overlap || c->n_cones == 0) && !std::getenv("AXG_NO_GRAPH"))
+    if (!prof.on && n >= AXG_GRAPH_MIN_STEPS && (overlap || c->n_cones == 0))
         graphed = enqueue_steps_graph(c, n);
     if (graphed >= 0) launches = (uint64_t)graphed;
     else
