@@ -89,3 +89,28 @@ def test_arrival_fraction_over_8_seeds(axg):
         total += 32
     fg, fo = arrived[0] / total, arrived[1] / total
     assert abs(fg - fo) <= 0.02, (fg, fo)
+
+
+def test_steady_state_total_against_the_closed_form(axg):
+    """T5 on the CUDA path directly, at a size the oracle would need minutes for: a point source in an absorbing 64 x 48 x
+    40 box, sigma = 1, Q = 400 per step.  N_ss = Q tau(x0) with the walls moved outward by 0.5826 sigma (the eigenfunction
+    series of tests/test_oracle_diffusion.py) within 1 %; without the shift the prediction is several per cent off, so
+    a wrong boundary rule, a dropped emission or a wrong step variance would show."""
+    from test_oracle_diffusion import _tau_box
+    grid, D, Q = (64, 48, 40), 0.5, 400
+    src = (30.0, 26.0, 17.0)
+    g = pu.new_axg(axg, grid, D, Q, 2.0, 0.25, 0.1, 91)
+    g.set_capacity(400_000, 4)
+    g.add_source(*src, 0, 1, 0)
+    for _ in range(15):                            # burn-in: > 5 slowest-mode time constants (L~^2 / (3 pi^2 D) = 290);
+        g.step(100)                                # in pieces: a call must fit n_live + n x Q into the capacity
+    tot, samples = 0, 600
+    for _ in range(samples):
+        g.step(10)
+        tot += g.counters()["n_live"]
+    n_ss = tot / samples
+    g.close()
+    tau = _tau_box(src, tuple(float(v) for v in grid), D, 1.0)
+    assert abs(n_ss / (Q * tau) - 1.0) < 0.01, (n_ss, Q * tau)
+    tau0 = _tau_box(src, tuple(float(v) for v in grid), D, 0.0)
+    assert abs(n_ss / (Q * tau0) - 1.0) > 0.03
