@@ -92,7 +92,8 @@ struct axg_ctx {
     size_t cells() const { return (size_t)grid.nx * grid.ny * grid.nz; }
     // cell arrays are padded to whole scan tiles so that 128-bit accesses of the last tile stay inside
     size_t cells_padded() const { return ((cells() + 1 + AXG_SCAN_TILE - 1) / AXG_SCAN_TILE + 1) * AXG_SCAN_TILE; }
-    size_t scan_tiles() const { return cells_padded() / AXG_SCAN_TILE + 2; }
+    // look-back words of k_cell_scan (one per tile) / block sums of k_cell_scan2 (one per block, at most 148 x 2)
+    size_t scan_tiles() const { return std::max<size_t>(cells_padded() / AXG_SCAN_TILE + 2, 512); }
 };
 
 namespace {

@@ -5,8 +5,9 @@
 // Why it exists: on B200 the radix passes are issue-bound, not HBM-bound (profiles/), while the array of per-cell
 // counts (4 B x cells: 67 MB at C3) sits in the 126 MB L2.  So P1 counts particles per cell with one L2 atomic each,
 // and P2 is
-//   k_cell_scan  cell_lo = exclusive scan of cnt over the cells (single pass, decoupled look-back)  -> O6 for free;
-//                cnt is re-zeroed on the way
+//   k_cell_scan2 cell_lo = exclusive scan of cnt over the cells (block sums, grid barrier, scan; cooperative launch)
+//                -> O6 for free; cnt is re-zeroed on the way.  k_cell_scan (single pass, decoupled look-back) is the
+//                fallback where a cooperative launch is not available
 //   k_place      slot[cell_lo[key] + arrival rank] = pre-sort row (| species << 30): cells are contiguous, the order
 //                INSIDE a cell is the arbitrary order in which P1's counting atomics arrived (they return the rank)
 //   k_settle     every slot finds its rank among the members of its cell by pre-sort index (the order std::stable_sort
@@ -20,7 +21,7 @@ namespace {
 
 // ---- exclusive scan of cnt[0 .. cells] --------------------------------------------------------------------------
 constexpr int SCAN_THREADS = 512;
-constexpr int SCAN_ITEMS = AXG_SCAN_TILE / SCAN_THREADS;  // 32 consecutive cells per thread: 8 x 128-bit
+constexpr int SCAN_ITEMS = AXG_SCAN_TILE / SCAN_THREADS;  // 16 consecutive cells per thread: 4 x 128-bit
 constexpr int SCAN_WARPS = SCAN_THREADS / 32;
 
 __global__ void __launch_bounds__(SCAN_THREADS) k_cell_scan(const AxgParams p) {
@@ -39,7 +40,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_cell_scan(const AxgParams p) {
         const uint32_t tile = s_tile;
         if (tile >= n_tiles) break;
         // the arrays are padded to a whole tile (zeros in cnt), so the vector accesses never leave them.  Every warp
-        // owns 1024 consecutive cells; chunk c of a lane is the 4 cells at (32 c + lane) * 4: each load and store
+        // owns 512 consecutive cells; chunk c of a lane is the 4 cells at (32 c + lane) * 4: each load and store
         // instruction of the warp covers 512 contiguous bytes.
         const size_t at4 = ((size_t)tile * AXG_SCAN_TILE + (size_t)warp * (32 * SCAN_ITEMS)) / 4 + lane;
         uint4 v[SCAN_ITEMS / 4];
@@ -100,6 +101,116 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_cell_scan(const AxgParams p) {
         dev->ticket = 0u;
         dev->done = 0u;
         dev->epoch = epoch + 1u;
+    }
+}
+
+// ---- the same scan without a chain: reduce, grid barrier, scan ------------------------------------------------------
+// In k_cell_scan 59 % of the stall samples sit at the barrier behind the look-back: 1 025 tiles chained through 296
+// resident blocks.  Here every block owns a CONTIGUOUS run of tiles: it sums them (phase 1), all blocks meet at a grid
+// barrier, every block adds up the sums of the blocks before it and scans its own run (phase 2, cnt re-read from the
+// L2).  Needs all blocks co-resident (2 per SM: axg_launch_cell_scan checks the occupancy and falls back otherwise).
+constexpr int SCAN2_BLOCKS_PER_SM = 2;
+
+__global__ void __launch_bounds__(SCAN_THREADS, SCAN2_BLOCKS_PER_SM) k_cell_scan2(const AxgParams p) {
+    __shared__ uint32_t s_warp[SCAN_WARPS];
+    __shared__ uint32_t s_red[SCAN_WARPS];
+    __shared__ uint32_t s_bcast;
+    AxgDev* dev = p.dev;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t G = gridDim.x, b = blockIdx.x;
+    const uint32_t gen = *(volatile uint32_t*)&dev->epoch;  // read before this block arrives at the barrier
+    const uint32_t n_el = p.cells + 1u;
+    const uint32_t n_tiles = (n_el + AXG_SCAN_TILE - 1) / AXG_SCAN_TILE;
+    const uint32_t per = (n_tiles + G - 1u) / G;
+    const uint32_t t0 = min(b * per, n_tiles), t1 = min(t0 + per, n_tiles);
+    const uint4* __restrict__ cnt4 = reinterpret_cast<const uint4*>(p.cnt);
+
+    // ---- phase 1: sum of my tiles ----
+    uint32_t acc = 0u;
+    for (uint32_t tile = t0; tile < t1; ++tile) {
+        const size_t at4 = (size_t)tile * (AXG_SCAN_TILE / 4) + tid;
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS / 4; ++k) {
+            const uint4 v = cnt4[at4 + (size_t)SCAN_THREADS * k];
+            acc += v.x + v.y + v.z + v.w;
+        }
+    }
+    acc = __reduce_add_sync(0xffffffffu, acc);
+    if (lane == 0) s_red[warp] = acc;
+    __syncthreads();
+    if (tid == 0) {
+        uint32_t total = 0u;
+        for (int w = 0; w < SCAN_WARPS; ++w) total += s_red[w];
+        axg_st_state(p.scan_state + b, (unsigned long long)total);
+        __threadfence();
+        if (atomicAdd(&dev->ticket, 1u) == G - 1u) {  // last to arrive: open the barrier
+            dev->ticket = 0u;
+            __threadfence();
+            atomicAdd(&dev->epoch, 1u);
+        } else {
+            while (*(volatile uint32_t*)&dev->epoch == gen) __nanosleep(64);
+        }
+        __threadfence();
+    }
+    __syncthreads();
+
+    // ---- phase 2: particles before my first tile, then the scan of my tiles ----
+    uint32_t before = 0u;
+    for (uint32_t i = tid; i < b; i += SCAN_THREADS) before += (uint32_t)axg_ld_state(p.scan_state + i);
+    before = __reduce_add_sync(0xffffffffu, before);
+    __syncthreads();
+    if (lane == 0) s_red[warp] = before;
+    __syncthreads();
+    if (tid == 0) {
+        uint32_t t = 0u;
+        for (int w = 0; w < SCAN_WARPS; ++w) t += s_red[w];
+        s_bcast = t;
+    }
+    __syncthreads();
+    uint32_t base = s_bcast;
+    for (uint32_t tile = t0; tile < t1; ++tile) {
+        const size_t at4 = ((size_t)tile * AXG_SCAN_TILE + (size_t)warp * (32 * SCAN_ITEMS)) / 4 + lane;
+        uint4 v[SCAN_ITEMS / 4];
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS / 4; ++k) v[k] = cnt4[at4 + 32 * k];
+        uint32_t pre[SCAN_ITEMS / 4];
+        uint32_t carry = 0u;
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS / 4; ++k) {
+            const uint32_t mine = v[k].x + v[k].y + v[k].z + v[k].w;
+            uint32_t incl = mine;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t u = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += u;
+            }
+            pre[k] = carry + incl - mine;
+            carry += __shfl_sync(0xffffffffu, incl, 31);
+        }
+        __syncthreads();  // s_warp of the previous tile has been read
+        if (lane == 31) s_warp[warp] = carry;
+        __syncthreads();
+        uint32_t woff = 0u, ttotal = 0u;
+#pragma unroll
+        for (int w = 0; w < SCAN_WARPS; ++w) {
+            const uint32_t c = s_warp[w];
+            woff += (w < warp) ? c : 0u;
+            ttotal += c;
+        }
+        const uint32_t wbase = base + woff;
+        const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS / 4; ++k) {
+            uint32_t run = wbase + pre[k];
+            uint4 o;
+            o.x = run; run += v[k].x;
+            o.y = run; run += v[k].y;
+            o.z = run; run += v[k].z;
+            o.w = run;
+            reinterpret_cast<uint4*>(p.cell_lo)[at4 + 32 * k] = o;
+            reinterpret_cast<uint4*>(p.cnt)[at4 + 32 * k] = zero;
+        }
+        base += ttotal;
     }
 }
 
@@ -177,6 +288,30 @@ __global__ void __launch_bounds__(SETTLE_THREADS, 8) k_settle(const AxgParams p)
 
 }  // namespace
 
-void axg_launch_cell_scan(const AxgParams& p, int grid, cudaStream_t s) { k_cell_scan<<<grid, SCAN_THREADS, 0, s>>>(p); }
+void axg_launch_cell_scan(const AxgParams& p, int grid, cudaStream_t s) {
+    static int resident = -1;  // blocks of k_cell_scan2 that fit one SM
+    if (resident < 0 &&
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, k_cell_scan2, SCAN_THREADS, 0) != cudaSuccess) {
+        cudaGetLastError();
+        resident = 0;
+    }
+    if (resident >= SCAN2_BLOCKS_PER_SM) {
+        // cooperative launch: the driver schedules all blocks of the grid together or not at all, so the grid barrier
+        // cannot deadlock against another context's kernels
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(148 * SCAN2_BLOCKS_PER_SM);
+        cfg.blockDim = dim3(SCAN_THREADS);
+        cfg.stream = s;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeCooperative;
+        attr[0].val.cooperative = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        if (cudaLaunchKernelEx(&cfg, k_cell_scan2, p) == cudaSuccess) return;
+        cudaGetLastError();
+        resident = 0;  // not supported here: the chained kernel from now on
+    }
+    k_cell_scan<<<grid, SCAN_THREADS, 0, s>>>(p);
+}
 void axg_launch_place(const AxgParams& p, int grid, cudaStream_t s) { k_place<<<grid, PLACE_THREADS, 0, s>>>(p); }
 void axg_launch_settle(const AxgParams& p, int grid, cudaStream_t s) { k_settle<<<grid, SETTLE_THREADS, 0, s>>>(p); }
