@@ -42,8 +42,8 @@ NOMINAL_GBS = 8000.0          # north_star's "~8 TB/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the `ncu --set full` capture
 # summarised in profiles/ (a capture is not repeatable inside a timed run, so it is a recorded number).
 TRAFFIC_NCU = {   # (workload, kernel) -> bytes per launch; profiles/r01_summary.md
-    ("C3", "k_diffuse_chunked"): 770.1e6, ("C3", "k_diffuse"): 578.9e6, ("C3", "k_settle"): 782.1e6,
-    ("C3", "k_place"): 266.5e6, ("C3", "k_cell_scan"): 142.9e6, ("C3", "k_sort_pass"): 203.7e6,
+    ("C3", "k_diffuse_chunked"): 771.3e6, ("C3", "k_diffuse"): 578.9e6, ("C3", "k_settle"): 781.6e6,
+    ("C3", "k_place"): 267.1e6, ("C3", "k_cell_scan2"): 173.3e6, ("C3", "k_sort_pass"): 203.7e6,
     ("C3", "k_reorder"): 740.8e6,
 }
 
@@ -321,7 +321,7 @@ def run_ours(args, w):
         step_bytes, bm, launches_of = bytes_model(w, n_avg, active, n_stencil, count_mode)
         per_step_ms = {k: v / K for k, v in ktimes.items()}
         kernel_name = {"diffuse": "k_diffuse_chunked" if count_mode else "k_diffuse", "sort": "k_sort_pass", "reorder": "k_reorder", "sense": "k_sense",
-                       "scan": "k_cell_scan", "place": "k_place", "settle": "k_settle"}
+                       "scan": "k_cell_scan2", "place": "k_place", "settle": "k_settle"}
         dom = max(bm.keys(), key=lambda k: per_step_ms[k])
         per_launch_ms = per_step_ms[dom] / launches_of[dom]
         per_launch_bytes = bm[dom] / launches_of[dom]
