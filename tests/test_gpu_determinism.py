@@ -129,3 +129,43 @@ def test_two_shards_on_one_gpu_equal_the_unsharded_run(axg):
     assert c[0]["next_id"] == c[1]["next_id"] == ref.counters()["next_id"]
     for g in shards + [ref]:
         g.close()
+
+
+def test_sharded_stepper_with_a_real_nccl_all_reduce(axg):
+    """The multi-GPU loop of paper_1405_3331_b200/sharded.py exactly as bench.py --gpus N runs it -- ShardedStepper, the
+    NCCL all-reduce on the ctx-owned device buffer wrapped without a copy, no host synchronisation inside -- with a
+    process group of ONE rank (the box has one GPU): must equal axg_step bit for bit."""
+    import os
+    import torch
+    import torch.distributed as dist
+    from paper_1405_3331_b200 import sharded as S
+
+    os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+    os.environ.setdefault("MASTER_PORT", "29571")
+    own_group = not dist.is_initialized()
+    if own_group:
+        dist.init_process_group("nccl", rank=0, world_size=1)
+    try:
+        w = W.small(seed=53, grid=(40, 33, 21), n_cones=200, n_sources=5, rate=150)
+        w.max_particles = 1 << 17
+
+        def make():
+            g = axg.Axg(w.grid, w.D, w.emission, w.radius, w.speed, w.noise, w.seed)
+            g.set_binning(axg.BIN_COUNT)
+            W.apply(g, w)
+            return g
+
+        ref, g = make(), make()
+        ref.step(25)
+        st = S.ShardedStepper(g, 0, 1, S.nccl_exchange)
+        st._exchange = S.nccl_exchange(g)   # with one rank the stepper would skip the exchange: force it
+        st.step(25)
+        torch.cuda.synchronize()
+        for f in FIELDS:
+            a, b = ref.read_state(f), g.read_state(f)
+            assert np.array_equal(a.view(np.uint8), b.view(np.uint8)), f
+        ref.close()
+        g.close()
+    finally:
+        if own_group:
+            dist.destroy_process_group()
