@@ -81,9 +81,10 @@ def bytes_model(w, n_live, n_active_cones, n_stencil, count_mode):
     sense = float(per_cone) * n_active_cones
     step = (38.0 + 12.0 + 16.0 * (passes - 1) + 42.0) * n_live + 8.0 * w.cells + sense
     if count_mode:
-        k = {"diffuse": (38.0 + 8.0) * n_live,    # + the 4 B counting atomic on cnt[key] and the 4 B arrival rank it returns
+        k = {"diffuse": (37.0 + 8.0) * n_live,    # 17 read + record 16 + key 4, + the 4 B counting atomic on cnt[key] and
+                                                   # the 4 B arrival rank it returns (the species byte rides in its top bits)
              "scan": 12.0 * (w.cells + 1),         # read cnt, write cell_lo, re-zero cnt
-             "place": 17.0 * n_live,               # key 4 + species 1 + arrival rank 4 + cell start 4 + slot 4
+             "place": 16.0 * n_live,               # key 4 + arrival rank | species 4 + cell start 4 + slot 4
              "settle": 53.0 * n_live,              # slot 4 + record 16 + cell_lo 8 + SoA 17 + key 4 + perm 4
              "sense": sense}
         launches = {"diffuse": 1, "scan": 1, "place": 1, "settle": 1, "sense": 1}

@@ -229,8 +229,8 @@ __global__ void __launch_bounds__(PLACE_THREADS) k_place(const AxgParams p) {
     for (uint32_t o = blockIdx.x * PLACE_THREADS + threadIdx.x; o < n_pp; o += gridDim.x * PLACE_THREADS) {
         if (o < n_phys && (o % AXG_CHUNK) >= __ldg(p.chunk_cnt + o / AXG_CHUNK)) continue;  // a hole
         const uint32_t k = __ldg(p.key_pre + o);
-        const uint32_t sp = __ldg(p.Bsp + o);
-        slot[__ldg(cell_lo + k) + __ldg(p.arr_pre + o)] = o | (sp << 30);
+        const uint32_t a = __ldg(p.arr_pre + o);  // arrival rank | species << 30
+        slot[__ldg(cell_lo + k) + (a & AXG_IDX_MASK)] = o | (a & ~AXG_IDX_MASK);
     }
 }
 

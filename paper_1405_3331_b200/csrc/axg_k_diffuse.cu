@@ -18,9 +18,11 @@ constexpr int DIFF_WARPS = DIFF_THREADS / 32;
 
 // What P1 leaves for P2 besides the key: radix mode -- the digit histograms of every pass (shared memory, flushed
 // once per block); count mode -- one more particle in cnt[key] (L2 reduction, no return value).
-__device__ __forceinline__ void tally(const AxgParams& p, uint32_t (*s_hist)[AXG_RADIX], uint32_t key, uint32_t o) {
+__device__ __forceinline__ void tally(const AxgParams& p, uint32_t (*s_hist)[AXG_RADIX], uint32_t key, uint32_t o,
+                                      uint32_t species) {
     if (p.bin_mode == AXG_BIN_COUNT_D) {
-        p.arr_pre[o] = atomicAdd(p.cnt + key, 1u);  // the old count = this row's arrival rank inside its cell
+        // the old count = this row's arrival rank inside its cell; the species rides in its top two bits (no Bsp column)
+        p.arr_pre[o] = atomicAdd(p.cnt + key, 1u) | (species << 30);
     } else {
 #pragma unroll
         for (int q = 0; q < AXG_MAX_PASSES; ++q)
@@ -61,10 +63,10 @@ __device__ void emit_and_close(const AxgParams& p, int do_emit, uint32_t (*s_his
             const uint32_t o = n_phys + e;
             const uint32_t key = axg_cell_key(p, sd.x, sd.y, sd.z);
             p.Brec[o] = make_float4(sd.x, sd.y, sd.z, __uint_as_float(next_id + p.src_id_prefix[s] + j));
-            p.Bsp[o] = (uint8_t)(sd.species_polarity & 0xffu);
+            if (p.bin_mode != AXG_BIN_COUNT_D) p.Bsp[o] = (uint8_t)(sd.species_polarity & 0xffu);
             p.key_pre[o] = key;
             if (p.bin_mode != AXG_BIN_COUNT_D) {
-                tally(p, s_hist, key, o);
+                tally(p, s_hist, key, o, 0u);
             } else if (j == 0u) {  // all newborns of a source share its cell: one atomic per source, not per particle
                 p.src_arr[s] = atomicAdd(p.cnt + key, p.src_emit_prefix[s + 1] - p.src_emit_prefix[s]);
             }
@@ -78,7 +80,7 @@ __device__ void emit_and_close(const AxgParams& p, int do_emit, uint32_t (*s_his
                 const uint32_t mid = (lo + hi) >> 1;
                 if (p.src_emit_prefix[mid] <= e) lo = mid; else hi = mid;
             }
-            p.arr_pre[n_phys + e] = p.src_arr[lo] + (e - p.src_emit_prefix[lo]);
+            p.arr_pre[n_phys + e] = (p.src_arr[lo] + (e - p.src_emit_prefix[lo])) | ((p.src[lo].species_polarity & 0xffu) << 30);
         }
     }
     if (p.bin_mode != AXG_BIN_COUNT_D) {
@@ -243,7 +245,7 @@ __global__ void __launch_bounds__(DIFF_THREADS, 4) k_diffuse(const AxgParams p) 
                 s_rec[o] = make_float4(x[i], y[i], z[i], __uint_as_float(id[i]));
                 s_sp[o] = (uint8_t)((sp_pack[i >> 2] >> (8 * (i & 3))) & 0xffu);
                 s_key[o] = key;
-                tally(p, s_hist, key, 0u);  // radix binning only: count binning runs k_diffuse_chunked
+                tally(p, s_hist, key, 0u, 0u);  // radix binning only: count binning runs k_diffuse_chunked
             }
             out += __popc(b);
         }
@@ -341,14 +343,14 @@ __global__ void __launch_bounds__(DIFF_THREADS, AXG_CHUNKED_BLOCKS) k_diffuse_ch
                 const uint32_t key = axg_cell_key(p, x[i], y[i], z[i]);
                 arr[i] = atomicAdd(p.cnt + key, 1u);  // old count = arrival rank inside the cell (see tally)
                 p.Brec[dst[i]] = make_float4(x[i], y[i], z[i], __uint_as_float(id[i]));
-                p.Bsp[dst[i]] = (uint8_t)sp[i];
                 p.key_pre[dst[i]] = key;
             }
             out += __popc(b);
         }
 #pragma unroll
         for (int i = 0; i < DIFF_ITEMS; ++i)  // the four atomics have been in flight together: one wait, not four
-            if ((alive >> i) & 1u) p.arr_pre[dst[i]] = arr[i];  // (storing them a trip later gains nothing: measured)
+            if ((alive >> i) & 1u) p.arr_pre[dst[i]] = arr[i] | (sp[i] << 30);  // species in the top two bits; (storing
+                                                                                // them a trip later gains nothing: measured)
         if (lane == 0) {
             const uint32_t c = out - chunk * AXG_CHUNK;
             p.chunk_cnt[chunk] = c;
@@ -376,10 +378,11 @@ __global__ void __launch_bounds__(256) k_rekey(const AxgParams p) {
         const float x = p.A.x[g], y = p.A.y[g], z = p.A.z[g];
         const uint32_t key = axg_cell_key(p, x, y, z);
         p.Brec[g] = make_float4(x, y, z, __uint_as_float(p.A.id[g]));
-        p.Bsp[g] = p.A.species[g];
+        const uint32_t sp = p.A.species[g];
+        if (p.bin_mode != AXG_BIN_COUNT_D) p.Bsp[g] = (uint8_t)sp;
         p.key_pre[g] = key;
         if (p.bin_mode == AXG_BIN_COUNT_D && (g % AXG_CHUNK) == 0u) p.chunk_cnt[g / AXG_CHUNK] = min(AXG_CHUNK, n - g);
-        tally(p, s_hist, key, g);
+        tally(p, s_hist, key, g, sp);
     }
     __syncthreads();
     for (int i = threadIdx.x; i < p.n_pass * AXG_RADIX; i += blockDim.x) {
