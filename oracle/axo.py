@@ -50,6 +50,7 @@ def lib():
         L.axo_add_source.argtypes = [vp, f32, f32, f32, C.c_uint8, C.c_int8, u32]
         L.axo_set_shard.argtypes = [vp, u32, u32]
         L.axo_set_steering.argtypes = [vp, C.c_int, f32, f32]
+        L.axo_set_sensing.argtypes = [vp, C.c_int]
         L.axo_step.argtypes = [vp, u32]
         L.axo_step_phase.argtypes = [vp, u32]
         L.axo_load_particles.argtypes = [vp, vp, vp, vp, vp, vp, u64, u32, u32]
@@ -112,6 +113,9 @@ class Oracle:
 
     def set_steering(self, mode, gain=1.0, turn=3.141592653589793 / 30):
         self._chk(self._L.axo_set_steering(self._h, int(mode), gain, turn))
+
+    def set_sensing(self, mode):
+        self._chk(self._L.axo_set_sensing(self._h, int(mode)))
 
     def set_shard(self, rank, world):
         self._chk(self._L.axo_set_shard(self._h, rank, world))

@@ -12,7 +12,9 @@
 // Pins (tests/test_oracle_*.py, all `-m "not gpu"`): T1 Philox known-answer vectors; T1b worked examples;
 // T2 moments of the normals; T3 conservation; T4 MSD = 6 D t; T5/T6 closed-form steady state of a point source
 // in an absorbing box; T7 Table 1 of the paper; T8 binning invariants vs numpy stable argsort; T9 grid sensing ==
-// brute force + planted linear gradient; T10 advance geometry and E[theta^2] = 2 noise^2; T11 append.
+// brute force + planted linear gradient; T10 advance geometry and E[theta^2] = 2 noise^2; T11 append; T13 the
+// fixed-turn steering rule (A-25); T14 per-particle sensing (A-26): worked example, reduction to the per-cell rule,
+// closed forms for a planted linear density, mirror / translation / order invariants.
 // PARITY UNPINNED: the absolute arrival fraction (T12) has no closed form; only GPU-vs-oracle agreement is tested.
 //
 // Build: g++ -O2 -std=c++17 -ffp-contract=off -shared -fPIC  (oracle/build.py)
@@ -118,6 +120,10 @@ struct axo_ctx {
     int steer_mode = 0;
     float snr_gain = 1.0f, cos_turn = 1.0f, sin_turn = 0.0f;
     uint32_t n_stencil = 0;  // |N_R|, filled by axo_set_steering
+    // sensing rule of P3: 0 = per cell (north_star, O7), 1 = per particle, 2 = per particle with distance weighting
+    // (section 5.3; reading A-26)
+    int sense_mode = 0;
+    int64_t moment_scale() const { return sense_mode == 0 ? 1 : 256; }  // units of M: cells (mode 0), 1/256 cell
 
     std::vector<Source> sources;
     int8_t species_polarity[MAX_SPECIES] = {0, 0, 0, 0};
@@ -264,11 +270,54 @@ void finish_gradient(axo_ctx* c, size_t cone, int64_t G[3]) {
         for (int a = 0; a < 3; ++a)
             G[a] += (int64_t)c->species_polarity[s] * c->cone_moment[(cone * MAX_SPECIES + s) * 3 + a];
     const int r2 = (int)std::floor((double)c->radius * (double)c->radius);
-    const float s2 = (float)stencil_S2(r2);
+    const float s2 = (float)(stencil_S2(r2) * c->moment_scale());
     for (int a = 0; a < 3; ++a) c->cone_gradient[cone * 3 + a] = (float)G[a] / s2;
 }
 
+// ---- P3, per-particle rule (section 5.3: "each individual particle that the axon's growth cone detects
+// would influence the axon's path"; reading A-26).  The plain definition: every active cone against every
+// particle, no grid.  A particle at x is detected by the cone at p iff |x - p|^2 <= R^2, the test taken in fp32 in
+// the order written here (a floating-point number decides an integer, so both implementations take the decision in
+// the same precision); a detected particle adds its offset from the cone, in fixed point, to the first moment of its
+// species:
+//    mode 1:  M_s += rint(256 * (x - p))                                  (units of 1/256 cell)
+//    mode 2:  M_s += rint(16 * w) * rint(16 * (x - p)),  w = 1 - d^2/R^2  (weight falling with the distance; same units)
+// rint = round to nearest, ties to even.  The sums are integers, hence independent of the summation order and
+// additive over disjoint particle sets (the sharded loop's all-reduce applies unchanged).
+void phase_sense_particles(axo_ctx* c) {
+    const float R2 = c->radius * c->radius;
+    for (size_t cone = 0; cone < c->n_cones(); ++cone) {
+        if (c->cone_state[cone] != CONE_ACTIVE) continue;  // A-16
+        const float px = c->cone_pos[cone * 3 + 0], py = c->cone_pos[cone * 3 + 1], pz = c->cone_pos[cone * 3 + 2];
+        int64_t* n = &c->cone_counts[cone * MAX_SPECIES];
+        int64_t* M = &c->cone_moment[cone * MAX_SPECIES * 3];
+        std::fill(n, n + MAX_SPECIES, 0);
+        std::fill(M, M + MAX_SPECIES * 3, 0);
+        for (size_t j = 0; j < c->A.size(); ++j) {
+            const float dx = c->A.x[j] - px, dy = c->A.y[j] - py, dz = c->A.z[j] - pz;
+            const float d2 = (dx * dx + dy * dy) + dz * dz;
+            if (!(d2 <= R2)) continue;
+            const int s = c->A.species[j];
+            n[s] += 1;
+            if (c->sense_mode == 1) {
+                M[s * 3 + 0] += (int64_t)std::nearbyint(dx * 256.0f);
+                M[s * 3 + 1] += (int64_t)std::nearbyint(dy * 256.0f);
+                M[s * 3 + 2] += (int64_t)std::nearbyint(dz * 256.0f);
+            } else {
+                const float w = 1.0f - d2 / R2;
+                const int64_t wq = (int64_t)std::nearbyint(w * 16.0f);
+                M[s * 3 + 0] += wq * (int64_t)std::nearbyint(dx * 16.0f);
+                M[s * 3 + 1] += wq * (int64_t)std::nearbyint(dy * 16.0f);
+                M[s * 3 + 2] += wq * (int64_t)std::nearbyint(dz * 16.0f);
+            }
+        }
+        int64_t G[3];
+        finish_gradient(c, cone, G);
+    }
+}
+
 void phase_sense(axo_ctx* c) {
+    if (c->sense_mode != 0) { phase_sense_particles(c); return; }
     if (c->cell_start.size() != c->cells()) {  // nothing binned yet: all cells empty
         c->cell_start.assign(c->cells(), 0u);
         c->cell_end.assign(c->cells(), 0u);
@@ -342,8 +391,8 @@ void phase_advance(axo_ctx* c) {
             const bool have_g = !(G[0] == 0 && G[1] == 0 && G[2] == 0);
             if (have_g && n_all > 0 && sinphi > 0.0f) {
                 const float gx = (float)G[0], gy = (float)G[1], gz = (float)G[2];
-                const float glen = std::sqrt(gx * gx + gy * gy + gz * gz) / (float)stencil_S2(
-                                       (int)std::floor((double)c->radius * (double)c->radius));
+                const float glen = std::sqrt(gx * gx + gy * gy + gz * gz) / (float)(c->moment_scale() * stencil_S2(
+                                       (int)std::floor((double)c->radius * (double)c->radius)));
                 const float gamma = (float)n_all / (float)c->n_stencil;
                 const float mu = glen / gamma;
                 const float one = 1.0f + gamma;
@@ -511,6 +560,13 @@ AXO_API int axo_add_source(axo_ctx* c, float x, float y, float z, uint8_t specie
 AXO_API int axo_set_shard(axo_ctx* c, uint32_t rank, uint32_t world) {
     if (!c || world == 0 || rank >= world) return fail(c, EINVAL_, "bad shard");
     c->shard_rank = rank; c->shard_world = world;
+    return OK;
+}
+
+// mode 0 = per cell (default), 1 = per particle, 2 = per particle, weighted by 1 - d^2/R^2 (reading A-26)
+AXO_API int axo_set_sensing(axo_ctx* c, int mode) {
+    if (!c || mode < 0 || mode > 2) return fail(c, EINVAL_, "bad sensing mode");
+    c->sense_mode = mode;
     return OK;
 }
 
