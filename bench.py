@@ -253,6 +253,8 @@ def run_ours(args, w):
     sim = W.prerun(make_sim, w, coarse=args.coarse)
     if args.steering == "snr":
         sim.set_steering(axg.STEER_SNR, 8.0, np.pi / 30)
+    if args.sensing != "cell":
+        sim.set_sensing(axg.SENSE_PARTICLE if args.sensing == "particle" else axg.SENSE_PARTICLE_WEIGHTED)
     if world > 1:
         step = sharded.ShardedStepper(sim, rank, world, sharded.nccl_exchange).step
     else:
@@ -415,7 +417,8 @@ def run_ours(args, w):
                        "l2": "inputs larger than L2 (particle SoA + sort buffers = %.0f MB per step)" % (
                            (2 * 17 + 20) * n_end / 1e6),
                        "parallelism": "shard-by-source x%d + int all-reduce" % world if world > 1 else "1 GPU",
-                       "prerun": "coarse-time x%d + 100 relax steps" % args.coarse, "steering": args.steering},
+                       "prerun": "coarse-time x%d + 100 relax steps" % args.coarse, "steering": args.steering,
+                       "sensing": args.sensing},
             "clocks": clock_rec, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "cpu_baseline": cpu,
             "cones": {k: cnt[k] for k in ("active", "arrived", "exited")},
         }
@@ -438,6 +441,8 @@ def main():
     ap.add_argument("--binning", default="auto", choices=("auto", "radix", "count"))
     ap.add_argument("--steering", default="vector", choices=("vector", "snr"),
                     help="P4 rule: north_star's vector addition, or the paper's fixed turn by the sign of N(SNR, 1)")
+    ap.add_argument("--sensing", default="cell", choices=("cell", "particle", "weighted"),
+                    help="P3 rule: north_star's per-cell sums, or the per-particle rule of the paper's section 5.3")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     from paper_1405_3331_b200 import workloads as W

@@ -195,6 +195,21 @@ int axg_set_binning(axg_ctx* ctx, int mode);
 enum { AXG_STEER_VECTOR = 0, AXG_STEER_SNR = 1 };
 int axg_set_steering(axg_ctx* ctx, int mode, float gain, float turn);
 
+/* Sensing rule of P3 (section 5.3: "each individual particle that the axon's
+ * growth cone detects would influence the axon's path"; reading A-26).
+ *  AXG_SENSE_CELL (default)  north_star's rule: counts and first moments over the CELLS of the index-space ball.
+ *  AXG_SENSE_PARTICLE        every particle at x with |x - p|^2 <= R^2 of the cone at p (fp32: d = x - p per axis,
+ *                            d2 = (dx*dx + dy*dy) + dz*dz, each operation rounded once, compared with fl(R*R)) counts 1
+ *                            and adds rint(256 d) per axis to the first moment of its species.
+ *  AXG_SENSE_PARTICLE_WEIGHTED  the same test; the particle adds rint(16 w) * rint(16 d) with w = 1 - d2 / fl(R*R):
+ *                            near particles weigh more.
+ * rint = round to nearest even.  Under both particle rules AXG_CONE_MOMENT is in units of 1/256 cell and
+ * AXG_CONE_GRADIENT = G / (256 S2(R)); the sums stay integers (bit-exact, additive over shards, same sense buffer and
+ * all-reduce), and P4 / P5 are unchanged.  Per cone the sums are int32 on the device: fewer than 2.7 M particles in
+ * range.  Needs the binned state of P2 like the cell rule.  May be called between any two steps; bad mode: AXG_EINVAL. */
+enum { AXG_SENSE_CELL = 0, AXG_SENSE_PARTICLE = 1, AXG_SENSE_PARTICLE_WEIGHTED = 2 };
+int axg_set_sensing(axg_ctx* ctx, int mode);
+
 /* Device pointer (int32[C][AXG_MAX_SPECIES][4] = n,Mx,My,Mz) of the per-cone sensing sums, for the NCCL
  * all-reduce between P3 and P4 when sharded.  *bytes = its size.  Owned by ctx.                           */
 int axg_sense_buffer(axg_ctx* ctx, void** device_ptr, size_t* bytes);

@@ -29,6 +29,7 @@ COUNTER_NAMES = ("step", "n_live", "next_id", "emitted", "absorbed", "active", "
 KERNEL_NAMES = ("clear", "diffuse", "emit", "sort", "reorder", "sense", "advance", "commit", "scan", "place", "settle")
 BIN_AUTO, BIN_RADIX, BIN_COUNT = 0, 1, 2
 STEER_VECTOR, STEER_SNR = 0, 1
+SENSE_CELL, SENSE_PARTICLE, SENSE_PARTICLE_WEIGHTED = 0, 1, 2
 AUTO_COUNT_MAX_CELLS = 1 << 31   # include/axg.h AXG_AUTO_COUNT_MAX_CELLS
 EXPORTS = (
     "axg_create", "axg_place_neurons", "axg_add_source", "axg_step", "axg_read_state", "axg_destroy",
@@ -36,6 +37,7 @@ EXPORTS = (
     "axg_sense_buffer", "axg_set_stream", "axg_set_allocator", "axg_last_step_stats", "axg_profile_next_step",
     "axg_kernel_times", "axg_check_capacity", "axg_enqueue_phase", "axg_sync", "axg_set_binning",
     "axg_set_steering",
+    "axg_set_sensing",
 )
 
 _ALLOC_T = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p)
@@ -87,6 +89,7 @@ def lib(build=True):
     L.axg_sync.argtypes = [vp]
     L.axg_set_binning.argtypes = [vp, C.c_int]
     L.axg_set_steering.argtypes = [vp, C.c_int, C.c_float, C.c_float]
+    L.axg_set_sensing.argtypes = [vp, C.c_int]
     L.axg_load_particles.argtypes = [vp, vp, vp, vp, vp, vp, u64, u32, u32]
     L.axg_load_cones.argtypes = [vp, vp, vp, vp, vp, u32]
     L.axg_read_state.argtypes = [vp, u32, vp, sz, C.POINTER(sz)]
@@ -185,6 +188,9 @@ class Axg:
 
     def set_binning(self, mode):
         self._chk(self._L.axg_set_binning(self._h, int(mode)))
+
+    def set_sensing(self, mode):
+        self._chk(self._L.axg_set_sensing(self._h, int(mode)))
 
     def set_steering(self, mode, gain=1.0, turn=3.141592653589793 / 30):
         self._chk(self._L.axg_set_steering(self._h, int(mode), gain, turn))

@@ -42,6 +42,7 @@ struct axg_ctx {
     uint64_t max_particles = 1ull << 20;
     uint32_t max_segments = 1024;
     uint32_t shard_rank = 0, shard_world = 1;
+    long long s2_cells = 0;  // S2(R) of the per-cell stencil (alloc_fixed)
     std::vector<Source> sources;
     int8_t species_polarity[AXG_MAX_SPECIES] = {0, 0, 0, 0};
     uint32_t n_cones = 0;
@@ -190,7 +191,10 @@ int alloc_fixed(axg_ctx* c) {
     P.src_emit_prefix = (const uint32_t*)c->d_src_emit_prefix;
     P.stencil = (const int32_t*)c->d_stencil;
     P.n_stencil = (uint32_t)st.size();
-    P.s2 = (float)s2;
+    c->s2_cells = s2;
+    P.s2 = (float)(s2 * (P.sense_mode ? 256 : 1));
+    P.radius = c->radius;
+    P.r2f = c->radius * c->radius;
     P.speed = c->speed; P.noise = c->noise;
     return AXG_OK;
 }
@@ -668,6 +672,14 @@ AXG_API int axg_set_steering(axg_ctx* c, int mode, float gain, float turn) {
     c->P.snr_gain = gain;
     c->P.cos_turn = (float)std::cos((double)turn);
     c->P.sin_turn = (float)std::sin((double)turn);
+    return AXG_OK;
+}
+
+AXG_API int axg_set_sensing(axg_ctx* c, int mode) {
+    if (!c || (mode != AXG_SENSE_CELL && mode != AXG_SENSE_PARTICLE && mode != AXG_SENSE_PARTICLE_WEIGHTED))
+        return fail(c, AXG_EINVAL, "bad sensing mode");
+    c->P.sense_mode = mode;
+    c->P.s2 = (float)(c->s2_cells * (mode ? 256 : 1));
     return AXG_OK;
 }
 

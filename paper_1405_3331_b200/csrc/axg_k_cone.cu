@@ -63,6 +63,105 @@ __global__ void __launch_bounds__(256) k_sense(const AxgParams p) {
     }
 }
 
+// ---- P3, per-particle rule (section 5.3; reading A-26; axg_set_sensing) ------------------
+// A particle at x is detected by the cone at q iff |x - q|^2 <= R^2 (fp32, operations and order fixed below); it adds
+// rint(256 (x - q)) -- or, weighted, rint(16 w) rint(16 (x - q)) with w = 1 - d^2 / R^2 -- to the first moment of its
+// species.  Integer sums: bit-exact, order-free, additive over shards.
+// One warp per cone.  The candidates are the particles of the cells that the ball can reach; in the sorted SoA the
+// cells x0..x1 of one (y, z) row are ONE contiguous run [cell_lo[key(x0, y, z)], cell_lo[key(x1, y, z) + 1]), so a lane
+// takes a row: two cell_lo loads and a short serial walk (~0.6 particles per cell away from the sources).  Rows with
+// AXG_PS_BIG or more particles (next to a source) are walked by the whole warp instead, 32 particles per request.
+// Rows and x ranges are clipped to the ball with a margin far above the fp32 rounding of the exact test, which alone
+// decides: the candidate set only has to be a superset.
+#define AXG_PS_BIG 24u
+
+__device__ __forceinline__ void axg_ps_add(const AxgParams& p, int (&acc)[AXG_MAX_SPECIES_D][4], uint32_t j, float qx,
+                                           float qy, float qz) {
+    const float dx = __fsub_rn(__ldg(p.A.x + j), qx), dy = __fsub_rn(__ldg(p.A.y + j), qy),
+                dz = __fsub_rn(__ldg(p.A.z + j), qz);
+    const float d2 = __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
+    if (!(d2 <= p.r2f)) return;
+    int mx, my, mz;
+    if (p.sense_mode == 1) {
+        mx = __float2int_rn(__fmul_rn(dx, 256.0f));
+        my = __float2int_rn(__fmul_rn(dy, 256.0f));
+        mz = __float2int_rn(__fmul_rn(dz, 256.0f));
+    } else {
+        const int wq = __float2int_rn(__fmul_rn(__fsub_rn(1.0f, __fdiv_rn(d2, p.r2f)), 16.0f));
+        mx = wq * __float2int_rn(__fmul_rn(dx, 16.0f));
+        my = wq * __float2int_rn(__fmul_rn(dy, 16.0f));
+        mz = wq * __float2int_rn(__fmul_rn(dz, 16.0f));
+    }
+    const int sp = (p.single_species >= 0) ? p.single_species : (int)__ldg(p.A.species + j);
+#pragma unroll
+    for (int s = 0; s < AXG_MAX_SPECIES_D; ++s)
+        if (s == sp) { acc[s][0] += 1; acc[s][1] += mx; acc[s][2] += my; acc[s][3] += mz; }
+}
+
+__global__ void __launch_bounds__(256) k_sense_particles(const AxgParams p) {
+    const int lane = threadIdx.x & 31;
+    const uint32_t warps_total = (gridDim.x * blockDim.x) >> 5;
+    const uint32_t* __restrict__ cell_lo = p.cell_lo;
+    const float Rm = p.radius * 1.00001f + 1e-5f;  // margin of the candidate box (not of the test)
+    for (uint32_t c = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; c < p.n_cones; c += warps_total) {
+        if (p.cone_state[c] != 0) {  // frozen cones skip P3..P5 (reading A-16)
+            if (p.sharded && lane < 16) p.sense[(size_t)c * 16 + lane] = 0;
+            continue;
+        }
+        const float qx = p.cone_pos[c * 3 + 0], qy = p.cone_pos[c * 3 + 1], qz = p.cone_pos[c * 3 + 2];
+        const int y0 = max(0, (int)floorf(qy - Rm)), y1 = min((int)p.ny - 1, (int)floorf(qy + Rm));
+        const int z0 = max(0, (int)floorf(qz - Rm)), z1 = min((int)p.nz - 1, (int)floorf(qz + Rm));
+        const int ny_rows = y1 - y0 + 1, n_rows = (y1 >= y0 && z1 >= z0) ? ny_rows * (z1 - z0 + 1) : 0;
+        int acc[AXG_MAX_SPECIES_D][4];
+#pragma unroll
+        for (int s = 0; s < AXG_MAX_SPECIES_D; ++s)
+#pragma unroll
+            for (int a = 0; a < 4; ++a) acc[s][a] = 0;
+        for (int r0 = 0; r0 < n_rows; r0 += 32) {
+            const int r = r0 + lane;
+            uint32_t a = 0, b = 0;
+            if (r < n_rows) {
+                const int y = y0 + r % ny_rows, z = z0 + r / ny_rows;
+                // squared distance from the cone to the slab of cells (y, z), then the half width left along x
+                const float ey = fmaxf(fmaxf((float)y - qy, qy - (float)(y + 1)), 0.0f);
+                const float ez = fmaxf(fmaxf((float)z - qz, qz - (float)(z + 1)), 0.0f);
+                const float left = Rm * Rm - (ey * ey + ez * ez);
+                if (left >= 0.0f) {
+                    const float hw = sqrtf(left) * 1.00001f + 1e-5f;
+                    const int x0 = max(0, (int)floorf(qx - hw)), x1 = min((int)p.nx - 1, (int)floorf(qx + hw));
+                    if (x1 >= x0) {
+                        const uint32_t row = ((uint32_t)z * p.ny + (uint32_t)y) * p.nx;
+                        a = __ldg(cell_lo + row + (uint32_t)x0);
+                        b = __ldg(cell_lo + row + (uint32_t)x1 + 1u);
+                    }
+                }
+            }
+            const bool big = (b - a) >= AXG_PS_BIG;
+            uint32_t bigs = __ballot_sync(0xffffffffu, big);
+            while (bigs) {  // crowded rows: the whole warp, coalesced
+                const int src = __ffs(bigs) - 1;
+                bigs &= bigs - 1;
+                const uint32_t ra = __shfl_sync(0xffffffffu, a, src), rb = __shfl_sync(0xffffffffu, b, src);
+                for (uint32_t j = ra + lane; j < rb; j += 32) axg_ps_add(p, acc, j, qx, qy, qz);
+            }
+            if (!big)
+                for (uint32_t j = a; j < b; ++j) axg_ps_add(p, acc, j, qx, qy, qz);
+        }
+        int mine = 0;
+        long long G[3] = {0, 0, 0};
+#pragma unroll
+        for (int s = 0; s < AXG_MAX_SPECIES_D; ++s)
+#pragma unroll
+            for (int a = 0; a < 4; ++a) {
+                const int v = __reduce_add_sync(0xffffffffu, acc[s][a]);
+                if (lane == s * 4 + a) mine = v;
+                if (a > 0) G[a - 1] += (long long)p.polarity[s] * v;
+            }
+        if (lane < 16) p.sense[(size_t)c * 16 + lane] = mine;
+        if (lane < 3) p.cone_gradient[c * 3 + lane] = (float)G[lane] / p.s2;
+    }
+}
+
 // ---- P4 + P5: one thread per cone ------------------------------------------------------------------------------
 // Every fp32 operation that the specification fixes is written with the explicit round-to-nearest intrinsics so
 // that nvcc cannot contract it into an fma (reading A-22); only the normals may differ by an ulp.
@@ -233,7 +332,10 @@ inline int grid_for(uint32_t n, int threads, int cap) {
 
 void axg_launch_sense(const AxgParams& p, cudaStream_t s) {
     if (!p.n_cones) return;
-    k_sense<<<grid_for(p.n_cones, 8, 148 * 8), 256, 0, s>>>(p);
+    if (p.sense_mode != 0)
+        k_sense_particles<<<grid_for(p.n_cones, 8, 148 * 8), 256, 0, s>>>(p);
+    else
+        k_sense<<<grid_for(p.n_cones, 8, 148 * 8), 256, 0, s>>>(p);
 }
 void axg_launch_advance(const AxgParams& p, int commit, cudaStream_t s) {
     if (!p.n_cones) return;

@@ -97,3 +97,36 @@ def test_one_step_against_the_oracle(c3):
     for f in ("CONE_POS", "CONE_HEADING"):
         assert pu.close(sim.read_state(f), o.read_state(f)).all()
     o.close()
+
+
+@pytest.mark.parametrize("mode", [1, 2])
+def test_particle_sensing_on_sampled_cones(c3, mode):
+    """Per-particle sensing (reading A-26) at full size: the oracle's all-pairs loop over the 16 M particles
+    for a sample of the active cones (the others are handed to it as frozen), bit for bit."""
+    m, w, sim = c3
+    sim.set_binning(m.BIN_AUTO)
+    sim.step(2)
+    a = _arrays(sim)
+    c = sim.counters()
+    state = sim.read_state("CONE_STATE")
+    active = np.flatnonzero(state == 0)
+    pick = np.random.default_rng(9 + mode).choice(active, min(10, len(active)), replace=False)
+    masked = np.full_like(state, 2)
+    masked[pick] = 0
+    o = axo.Oracle(w.grid, w.D, w.emission, w.radius, w.speed, w.noise, w.seed)
+    W.apply(o, w)
+    o.set_sensing(mode)
+    o.load_particles(a["X"], a["Y"], a["Z"], a["SPECIES"], a["ID"], next_id=c["next_id"], step=c["step"])
+    o.load_cones(sim.read_state("CONE_POS"), sim.read_state("CONE_HEADING"), masked, sim.read_state("POLY_LEN"))
+    o.step_phase(axo.PHASE_SENSE)
+    try:
+        sim.set_sensing(mode)
+        sim.step_phase(m.PHASE_SENSE)
+        gc = sim.read_state("CONE_COUNTS").reshape(-1, 4)[pick]
+        gm = sim.read_state("CONE_MOMENT").reshape(-1, 12)[pick]
+    finally:
+        sim.set_sensing(m.SENSE_CELL)
+    assert np.array_equal(gc, o.read_state("CONE_COUNTS").reshape(-1, 4)[pick])
+    assert np.array_equal(gm, o.read_state("CONE_MOMENT").reshape(-1, 12)[pick])
+    assert gc.sum() > 0
+    o.close()

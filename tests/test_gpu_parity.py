@@ -27,13 +27,16 @@ def axg(request):
     pu.BINNING = None
 
 
-def _chain(axg, w, n, seed, steps=2, n_species=2, steering=None):
+def _chain(axg, w, n, seed, steps=2, n_species=2, steering=None, sensing=None):
     """load -> [P1 | P2 | P3 | P4+P5] x steps, each phase compared; the oracle is re-fed the GPU's P1 output so that
     integer phases are compared on identical inputs."""
     g, o = make_pair(w, axg)
     if steering is not None:
         g.set_steering(*steering)
         o.set_steering(*steering)
+    if sensing is not None:
+        g.set_sensing(sensing)
+        o.set_sensing(sensing)
     load_same_particles(g, o, seed, n, w.grid, n_species=n_species, step=3)
     flips = 0
     for k in range(steps):
@@ -54,6 +57,11 @@ def _chain(axg, w, n, seed, steps=2, n_species=2, steering=None):
         g.step_phase(axg.PHASE_ADVANCE | axg.PHASE_COMMIT)
         o.step_phase(axo.PHASE_ADVANCE | axo.PHASE_COMMIT)
         compare_cones(g, o)
+        if sensing is not None:
+            # per-particle sensing takes x - p in fp32: its integers are compared on identical cone positions, as the
+            # binning is on identical particle positions (the positions agreed within tolerance just above)
+            o.load_cones(g.read_state("CONE_POS"), g.read_state("CONE_HEADING"), g.read_state("CONE_STATE"),
+                         g.read_state("POLY_LEN"))
     g.close()
     o.close()
     return flips
@@ -235,3 +243,59 @@ def test_chain_snr_steering(axg):
     for gain in (0.0, 8.0):
         w = W.small(seed=23, n_cones=400, grid=(24, 20, 16))
         _chain(axg, w, n=60_013, seed=29, steps=3, steering=(1, gain, math.pi / 30))
+
+
+@pytest.mark.parametrize("mode", [1, 2])
+def test_chain_particle_sensing(axg, mode):
+    """SURVEY.md §8(f) NEXT-2 (reading A-26): per-particle sensing, flat and weighted.  Counts
+    and fixed-point moments bit-exact against the oracle's all-pairs loop, then P4 / P5 on them within NS's tolerance."""
+    w = W.small(seed=31, n_cones=300, grid=(24, 20, 16))
+    _chain(axg, w, n=60_013, seed=37, steps=3, sensing=mode)
+    w = W.small(seed=32, grid=(40, 33, 21), n_cones=200, two_species=False, radius=3.0)
+    _chain(axg, w, n=30_011, seed=38, steps=2, n_species=1, sensing=mode)
+    import math
+    w = W.small(seed=33, n_cones=100, grid=(24, 20, 16), radius=2.5)
+    _chain(axg, w, n=20_001, seed=39, steps=2, sensing=mode, steering=(1, 8.0, math.pi / 30))
+
+
+@pytest.mark.parametrize("mode", [1, 2])
+def test_particle_sensing_on_given_state(axg, mode):
+    """P3 alone on identical particles and cones: cones in the corners, on the walls, on cell faces, inside a cell that
+    holds thousands of particles (the whole-warp path of k_sense_particles) and in empty space; particles exactly on
+    the sphere of a cone (d^2 == R^2: detected).  Bit-exact counts and moments."""
+    grid = (12, 10, 9)
+    n = 40_000
+    for R in (1.0, 2.0, 2.75):
+        g = pu.new_axg(axg, grid, 0.5, 1, R, 0.25, 0.1, 3)
+        o = axo.Oracle(grid, 0.5, 1, R, 0.25, 0.1, 3)
+        x, y, z, sp, ids = W.random_particles(5, n, grid, n_species=2)
+        k = int(n * 0.5)
+        for a, c in zip((x, y, z), (5.0, 4.0, 3.0)):
+            a[:k] = c + (a[:k] - np.floor(a[:k])) * 1.5
+        rng = np.random.default_rng(77)
+        nx, ny, nz = grid
+        hi = [np.nextafter(np.float32(v), np.float32(0)) for v in grid]
+        corners = [(a, b, c) for a in (0.0, hi[0]) for b in (0.0, hi[1]) for c in (0.0, hi[2])]
+        faces = [(3.0, 4.0, 5.0), (5.0, 4.0, 3.0), (6.5, 5.5, 4.5), (5.75, 4.75, 3.75), (0.25, 5.0, 8.75)]
+        rest = np.stack([rng.uniform(0, nx, 200), rng.uniform(0, ny, 200), rng.uniform(0, nz, 200)], 1)
+        cones = np.concatenate([np.array(corners), np.array(faces), rest], 0).astype(np.float32)
+        # particles exactly R away from the cone at (3, 4, 5) along each axis (R is dyadic: exact in fp32)
+        ring = np.array([[3 + R, 4, 5], [3, 4 + R, 5], [3, 4, 5 - R], [3 - R, 4, 5]], np.float32)
+        x[-4:], y[-4:], z[-4:] = ring[:, 0], ring[:, 1], ring[:, 2]
+        for s in (g, o):
+            s.set_capacity(n + 16, 4)
+            s.add_source(6.0, 5.0, 4.0, 0, 1, 1)
+            s.add_source(2.0, 2.0, 2.0, 1, -1, 1)
+            s.set_sensing(mode)
+            s.place_neurons(cones)
+            s.load_particles(x, y, z, sp, ids, next_id=n, step=0)
+        g.step_phase(axg.PHASE_BIN | axg.PHASE_SENSE)
+        o.step_phase(axo.PHASE_BIN | axo.PHASE_SENSE)
+        compare_binning(g, o)
+        compare_sense(g, o)
+        cnt = o.read_state("CONE_COUNTS").reshape(-1, 4)
+        if R >= 2:
+            assert cnt.sum(1).max() > 5000
+        assert cnt[8].sum() >= 4          # the four particles on the sphere of cone 8 are detected
+        g.close()
+        o.close()
