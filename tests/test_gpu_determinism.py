@@ -25,13 +25,14 @@ def axg():
     return m
 
 
-def _run(axg, binning, calls, steering=None):
+def _run(axg, binning, calls, steering=None, sensing=0):
     w = W.small(seed=41, grid=(40, 33, 21), n_cones=300, n_sources=4, rate=300)
     w.max_particles = 1 << 18
     g = axg.Axg(w.grid, w.D, w.emission, w.radius, w.speed, w.noise, w.seed)
     g.set_binning(binning)
     if steering:
         g.set_steering(*steering)
+    g.set_sensing(sensing)
     W.apply(g, w)
     x, y, z, sp, ids = W.random_particles(43, 120_007, w.grid, n_species=2)
     g.load_particles(x, y, z, sp, ids, next_id=len(ids), step=0)
@@ -69,12 +70,25 @@ def test_count_binning_equals_radix_binning(axg):
     _same(a, b)
 
 
+@pytest.mark.parametrize("sensing", [1, 2])
+def test_particle_sensing_is_deterministic(axg, sensing):
+    """per-particle sensing (reading A-26): graph replay vs single steps, count vs radix binning, byte for byte; and it
+    is not the per-cell rule in disguise (the cones end up elsewhere)."""
+    a = _run(axg, axg.BIN_COUNT, [STEPS], sensing=sensing)
+    _same(a, _run(axg, axg.BIN_COUNT, [1] * STEPS, sensing=sensing))
+    _same(a, _run(axg, axg.BIN_RADIX, [7, 1, 22], sensing=sensing))
+    cell = _run(axg, axg.BIN_COUNT, [STEPS])
+    assert not np.array_equal(a["CONE_POS"], cell["CONE_POS"])
+    assert np.array_equal(a["PART_ID"], cell["PART_ID"])      # the particles do not depend on the cones
+
+
 def test_count_equals_radix_with_the_fixed_turn_rule(axg):
     st = (1, 8.0, np.pi / 30)
     _same(_run(axg, axg.BIN_COUNT, [STEPS], st), _run(axg, axg.BIN_RADIX, [STEPS], st))
 
 
-def test_two_shards_on_one_gpu_equal_the_unsharded_run(axg):
+@pytest.mark.parametrize("sensing", [0, 1])   # per-cell rule; per-particle rule (integer sums too: reading A-26)
+def test_two_shards_on_one_gpu_equal_the_unsharded_run(axg, sensing):
     """DESIGN.md §8 on the real library: two contexts sharded by source (axg_set_shard, the enqueue / sync calls of the
     multi-GPU loop), the all-reduce replaced by a sum of the two device buffers on the same stream.  The cones must be
     bit-identical to the unsharded run, and the two shards' particles together must be its particles, bit for bit.
@@ -89,6 +103,7 @@ def test_two_shards_on_one_gpu_equal_the_unsharded_run(axg):
     def make():
         g = axg.Axg(w.grid, w.D, w.emission, w.radius, w.speed, w.noise, w.seed)
         g.set_binning(axg.BIN_COUNT)
+        g.set_sensing(sensing)
         W.apply(g, w)
         return g
 

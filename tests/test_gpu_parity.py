@@ -299,3 +299,39 @@ def test_particle_sensing_on_given_state(axg, mode):
         assert cnt[8].sum() >= 4          # the four particles on the sphere of cone 8 are detected
         g.close()
         o.close()
+
+
+@pytest.mark.parametrize("mode,coef", [(1, 4 / 15), (2, 8 / 105)])
+def test_particle_sensing_against_the_closed_form(axg, mode, coef):
+    """The CUDA path against the mathematics directly (no oracle): a cloud of density rho0 (1 + k . (x - centre)) gives
+    E[M] = 256 rho0 k coef pi R^5 (coef = 4/15 flat, 8/105 with the weight 1 - r^2/R^2) and E[n] = rho (4 pi / 3) R^3."""
+    grid = (16, 16, 16)
+    k = np.array([0.08, -0.04, 0.0])
+    n = 4_000_000
+    rng = np.random.default_rng(11)
+    parts = []
+    while sum(len(a) for a in parts) < n:
+        x = rng.uniform(0, 16, (n, 3))
+        parts.append(x[rng.uniform(0, 1.0 + np.abs(k).sum() * 8, n) < 1.0 + (x - 8.0) @ k])
+    pts = np.concatenate(parts)[:n].astype(np.float32)
+    pts = np.minimum(pts, np.nextafter(np.float32(16), np.float32(0)))
+    rho0 = n / 16.0 ** 3
+    c = np.array([[x, y, z] for x in (4.3, 6.6, 8.9, 11.2) for y in (4.1, 6.7, 9.0, 11.4) for z in (4.5, 6.9, 9.2, 11.0)],
+                 np.float32)
+    for R in (2.0, 3.0):
+        g = pu.new_axg(axg, grid, 0.5, 1, R, 0.25, 0.0, 1)
+        g.set_capacity(n + 16, 4)
+        g.add_source(1.0, 1.0, 1.0, 0, 1, 1)
+        g.set_sensing(mode)
+        g.place_neurons(c)
+        g.load_particles(pts[:, 0], pts[:, 1], pts[:, 2], np.zeros(n, np.uint8), np.arange(n, dtype=np.uint32),
+                         next_id=n, step=0)
+        g.step_phase(axg.PHASE_BIN | axg.PHASE_SENSE)
+        cnt = g.read_state("CONE_COUNTS").reshape(-1, 4)[:, 0]
+        M = g.read_state("CONE_MOMENT").reshape(-1, 4, 3)[:, 0, :].mean(0)
+        g.close()
+        expect = 256 * rho0 * k * coef * np.pi * R ** 5
+        assert abs(M[0] - expect[0]) < 0.05 * abs(expect[0]), (R, M, expect)
+        assert abs(M[1] - expect[1]) < 0.09 * abs(expect[1]), (R, M, expect)
+        assert abs(M[2]) < 0.05 * abs(expect[0]), (R, M, expect)
+        np.testing.assert_allclose(cnt, rho0 * (1 + (c.astype(np.float64) - 8.0) @ k) * 4 * np.pi / 3 * R ** 3, rtol=0.03)

@@ -30,10 +30,11 @@ def _workload():
     return w
 
 
-def _oracle(w):
+def _oracle(w, sensing=0):
     from oracle import axo
     from paper_1405_3331_b200 import workloads as W
     o = axo.Oracle(w.grid, w.D, w.emission, w.radius, w.speed, w.noise, w.seed)
+    o.set_sensing(sensing)
     return W.apply(o, w)
 
 
@@ -44,14 +45,14 @@ def _state(o):
     return out
 
 
-def _worker(rank, world, port, q):
+def _worker(rank, world, port, q, sensing):
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
         from paper_1405_3331_b200 import sharded
         w = _workload()
-        o = _oracle(w)
+        o = _oracle(w, sensing)
         stepper = sharded.ShardedStepper(o, rank, world, sharded.host_exchange)
         stepper.step(STEPS)
         st = _state(o)
@@ -69,16 +70,17 @@ def _free_port():
 
 
 @pytest.mark.timeout(300)
-def test_two_ranks_equal_the_unsharded_run():
+@pytest.mark.parametrize("sensing", [0, 2])   # per-cell rule; per-particle weighted rule (integer sums as well, A-26)
+def test_two_ranks_equal_the_unsharded_run(sensing):
     w = _workload()
-    ref = _oracle(w)
+    ref = _oracle(w, sensing)
     ref.step(STEPS)
     want = _state(ref)
 
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
     port = _free_port()
-    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q, sensing)) for r in range(2)]
     for p in procs:
         p.start()
     got = dict(q.get(timeout=240) for _ in range(2))
