@@ -85,7 +85,7 @@ def bytes_model(w, n_live, n_active_cones, n_stencil, count_mode):
                                                    # the 4 B arrival rank it returns (the species byte rides in its top bits)
              "scan": 12.0 * (w.cells + 1),         # read cnt, write cell_lo, re-zero cnt
              "place": 16.0 * n_live,               # key 4 + arrival rank | species 4 + cell start 4 + slot 4
-             "settle": 53.0 * n_live,              # slot 4 + record 16 + cell_lo 8 + SoA 17 + key 4 + perm 4
+             "settle": 45.0 * n_live,              # slot 4 + record 16 + cell_lo 8 + SoA 17 (keys / perm: derived on read)
              "sense": sense}
         launches = {"diffuse": 1, "scan": 1, "place": 1, "settle": 1, "sense": 1}
     else:

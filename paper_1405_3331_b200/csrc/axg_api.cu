@@ -71,6 +71,7 @@ struct axg_ctx {
     void* d_scan_state = nullptr;
     int bin_request = AXG_BIN_AUTO;
     bool b_chunked = false;   // the pre-sort array is in the chunked layout of k_diffuse_chunked (count binning)
+    bool kp_pending = false;  // count binning: the last P2 left sorted keys / permutation to be derived on read (k_settle<true>)
     bool cnt_dirty = false;   // P1 has counted into cnt and P2 has not consumed (and re-zeroed) it yet
     void* d_src = nullptr;
     void* d_src_id_prefix = nullptr;
@@ -391,6 +392,7 @@ int enqueue_phases(axg_ctx* c, uint32_t mask, Prof& prof, bool overlap = false) 
         launches += 1;
         c->cnt_dirty = count_mode;
         c->b_chunked = count_mode;
+        c->kp_pending = false;  // the records that a replay of k_settle would gather are gone
     }
     if (mask & AXG_PHASE_BIN) {
         // the previous step's P3 (side stream) still reads cell_lo and the species column that P2 rewrites
@@ -409,10 +411,12 @@ int enqueue_phases(axg_ctx* c, uint32_t mask, Prof& prof, bool overlap = false) 
             prof.mark(AXG_K_PLACE);
             axg_launch_place(P, N_SM * 8, s);
             prof.mark(AXG_K_SETTLE);
-            axg_launch_settle(P, N_SM * 8, s);
+            axg_launch_settle(P, N_SM * 8, 0, s);
             launches += 3;
             c->cnt_dirty = false;
+            c->kp_pending = true;
         } else {
+            c->kp_pending = false;
             prof.mark(AXG_K_SORT);
             for (int q = 0; q < P.n_pass; ++q) axg_launch_sort_pass(P, q, N_SM * 2, s);
             prof.mark(AXG_K_REORDER);
@@ -474,7 +478,7 @@ int enqueue_unit(axg_ctx* c, cudaStream_t s, bool prev_cones) {
     if (count_mode) {
         axg_launch_cell_scan(P, N_SM * 4, s);
         axg_launch_place(P, N_SM * 8, s);
-        axg_launch_settle(P, N_SM * 8, s);
+        axg_launch_settle(P, N_SM * 8, 0, s);
         launches += 4;
     } else {
         for (int q = 0; q < P.n_pass; ++q) axg_launch_sort_pass(P, q, N_SM * 2, s);
@@ -552,6 +556,7 @@ long long enqueue_steps_graph(axg_ctx* c, uint32_t n) {
     }
     c->cnt_dirty = false;
     c->b_chunked = c->P.bin_mode == AXG_BIN_COUNT_D;
+    c->kp_pending = c->b_chunked;
     return launches;
 }
 
@@ -769,6 +774,7 @@ AXG_API int axg_set_capacity(axg_ctx* c, uint64_t max_particles, uint32_t max_se
         c->particle_bufs = nb;
         c->particles_allocated = true;
         c->n_B = 0;
+        c->kp_pending = false;
     }
     c->max_particles = max_particles;
     return c->particles_allocated ? resolve_binning(c) : AXG_OK;  // AXG_BIN_AUTO depends on the capacity
@@ -806,6 +812,7 @@ AXG_API int axg_load_particles(axg_ctx* c, const float* x, const float* y, const
     CU(c, cudaMemcpyAsync(&d->pstep, &step, 4, cudaMemcpyHostToDevice, c->stream));
     CU(c, cudaStreamSynchronize(c->stream));
     c->n_A = n32;
+    c->kp_pending = false;  // A is new: nothing of the last P2 may be replayed
     c->loaded_species_mask = mask;
     return upload_sources(c);
 }
@@ -998,10 +1005,16 @@ AXG_API int axg_read_state(axg_ctx* c, uint32_t field, void* dst, size_t dst_byt
         case AXG_PART_Z: return copy_out(c, P.A.z, nA, 4, dst, dst_bytes, n_elems);
         case AXG_PART_SPECIES: return copy_out(c, P.A.species, nA, 1, dst, dst_bytes, n_elems);
         case AXG_PART_ID: return copy_out(c, P.A.id, nA, 4, dst, dst_bytes, n_elems);
-        case AXG_KEYS_SORTED: return copy_out(c, have_p ? P.skey[P.final_buf] : nullptr, nB, 4, dst, dst_bytes, n_elems);
+        case AXG_KEYS_SORTED:
         case AXG_PERM:
-            return export_out(c, nB, 4, dst, dst_bytes, n_elems,
-                              [&](void* t) { axg_launch_perm_export(P, c->b_chunked ? 1 : 0, (uint32_t*)t, c->stream); });
+            if (c->kp_pending) {  // count binning stores neither on the path: derive them now (see k_settle)
+                axg_launch_settle(P, N_SM * 8, 1, c->stream);
+                c->kp_pending = false;
+            }
+            if (field == AXG_PERM)
+                return export_out(c, nB, 4, dst, dst_bytes, n_elems,
+                                  [&](void* t) { axg_launch_perm_export(P, c->b_chunked ? 1 : 0, (uint32_t*)t, c->stream); });
+            return copy_out(c, have_p ? P.skey[P.final_buf] : nullptr, nB, 4, dst, dst_bytes, n_elems);
         case AXG_CELL_START:
             return export_out(c, c->cells(), 4, dst, dst_bytes, n_elems,
                               [&](void* t) { axg_launch_cell_export(P, (uint32_t*)t, nullptr, c->stream); });

@@ -240,6 +240,10 @@ constexpr int SETTLE_ITEMS = 1;  // warp-striped (item i of lane l is slot base 
                                  // 8 blocks per SM 0.188 ms, 2 items 0.198, 4 items / 6 blocks 0.227, 8 items 0.272 --
                                  // the kernel lives on many independent warps in flight, not on ILP inside one
 
+// WITH_KP: also store the sorted keys and the permutation.  Nothing on the path reads them (P1 recomputes the key, P3
+// works from cell_lo), so the step runs the lean kernel and axg_read_state(AXG_KEYS_SORTED / AXG_PERM) replays the
+// full one on the intact inputs (slot list, records, cell_lo): the same values land in the same places.
+template <bool WITH_KP>
 __global__ void __launch_bounds__(SETTLE_THREADS, 8) k_settle(const AxgParams p) {
     const uint32_t n = p.dev->n_live;
     const uint32_t* __restrict__ slot = p.sidx[p.final_buf ^ 1];
@@ -280,8 +284,10 @@ __global__ void __launch_bounds__(SETTLE_THREADS, 8) k_settle(const AxgParams p)
             p.A.z[dst] = r[i].z;
             p.A.id[dst] = __float_as_uint(r[i].w);
             p.A.species[dst] = (uint8_t)(v[i] >> 30);
-            keys[dst] = k;
-            perm[dst] = v[i];
+            if (WITH_KP) {
+                keys[dst] = k;
+                perm[dst] = v[i];
+            }
         }
     }
 }
@@ -314,4 +320,7 @@ void axg_launch_cell_scan(const AxgParams& p, int grid, cudaStream_t s) {
     k_cell_scan<<<grid, SCAN_THREADS, 0, s>>>(p);
 }
 void axg_launch_place(const AxgParams& p, int grid, cudaStream_t s) { k_place<<<grid, PLACE_THREADS, 0, s>>>(p); }
-void axg_launch_settle(const AxgParams& p, int grid, cudaStream_t s) { k_settle<<<grid, SETTLE_THREADS, 0, s>>>(p); }
+void axg_launch_settle(const AxgParams& p, int grid, int with_keys_perm, cudaStream_t s) {
+    if (with_keys_perm) k_settle<true><<<grid, SETTLE_THREADS, 0, s>>>(p);
+    else k_settle<false><<<grid, SETTLE_THREADS, 0, s>>>(p);
+}
