@@ -41,8 +41,8 @@ HBM_FALLBACK_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md "FALLBACK"
 NOMINAL_GBS = 8000.0          # north_star's "~8 TB/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the `ncu --set full` capture
 # summarised in profiles/ (a capture is not repeatable inside a timed run, so it is a recorded number).
-TRAFFIC_NCU = {   # (workload, kernel) -> bytes per launch; profiles/r01_summary.md
-    ("C3", "k_diffuse_chunked"): 753.7e6, ("C3", "k_diffuse"): 578.9e6, ("C3", "k_settle"): 783.0e6,
+TRAFFIC_NCU = {   # (workload, kernel) -> bytes per launch; profiles/r01_summary.md, r01c_summary.md
+    ("C3", "k_diffuse_chunked"): 753.7e6, ("C3", "k_diffuse"): 578.9e6, ("C3", "k_settle"): 652.7e6,
     ("C3", "k_place"): 248.8e6, ("C3", "k_cell_scan2"): 172.6e6, ("C3", "k_sort_pass"): 203.7e6,
     ("C3", "k_reorder"): 740.8e6,
 }
