@@ -51,6 +51,7 @@ def lib():
         L.axo_set_shard.argtypes = [vp, u32, u32]
         L.axo_set_steering.argtypes = [vp, C.c_int, f32, f32]
         L.axo_set_sensing.argtypes = [vp, C.c_int]
+        L.axo_set_key_order.argtypes = [vp, C.c_int]
         L.axo_step.argtypes = [vp, u32]
         L.axo_step_phase.argtypes = [vp, u32]
         L.axo_load_particles.argtypes = [vp, vp, vp, vp, vp, vp, u64, u32, u32]
@@ -113,6 +114,9 @@ class Oracle:
 
     def set_steering(self, mode, gain=1.0, turn=3.141592653589793 / 30):
         self._chk(self._L.axo_set_steering(self._h, int(mode), gain, turn))
+
+    def set_key_order(self, order):
+        self._chk(self._L.axo_set_key_order(self._h, int(order)))
 
     def set_sensing(self, mode):
         self._chk(self._L.axo_set_sensing(self._h, int(mode)))

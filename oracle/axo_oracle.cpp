@@ -146,7 +146,21 @@ struct axo_ctx {
     std::vector<float> poly;  // C*(max_segments+1)*3 neuron-major
 
     std::string err;
-    size_t cells() const { return (size_t)nx * ny * nz; }
+    // cell order ("a Z-order curve ... potential optimization"; reading A-27):
+    // 0 = linear, x fastest (north_star); 1 = bricks of 8 x 4 x 4 cells, bricks in linear order (x fastest), cells inside
+    // a brick in linear order (x fastest): key = brick * 128 + (z & 3) * 32 + (y & 3) * 8 + (x & 7).  The key space covers
+    // the grid padded to whole bricks.
+    int key_order = 0;
+    size_t cells() const {
+        if (key_order == 0) return (size_t)nx * ny * nz;
+        return (size_t)((nx + 7) / 8) * ((ny + 3) / 4) * ((nz + 3) / 4) * 128;
+    }
+    uint32_t key_of_cell(uint32_t ix, uint32_t iy, uint32_t iz) const {
+        if (key_order == 0) return (iz * ny + iy) * nx + ix;
+        const uint32_t nbx = (nx + 7) / 8, nby = (ny + 3) / 4;
+        const uint32_t brick = ((iz / 4) * nby + (iy / 4)) * nbx + (ix / 8);
+        return brick * 128 + (iz % 4) * 32 + (iy % 4) * 8 + (ix % 8);
+    }
     size_t n_cones() const { return cone_state.size(); }
 };
 
@@ -166,7 +180,7 @@ bool inside(const axo_ctx* c, float x, float y, float z) {
 
 // O3 (reading A-8; "calculateHash", linear id): truncation of non-negative fp32, x fastest.
 uint32_t cell_key(const axo_ctx* c, float x, float y, float z) {
-    return ((uint32_t)z * c->ny + (uint32_t)y) * c->nx + (uint32_t)x;
+    return c->key_of_cell((uint32_t)x, (uint32_t)y, (uint32_t)z);  // linear unless axo_set_key_order (A-27)
 }
 
 uint64_t owned_rate(const axo_ctx* c) {
@@ -338,7 +352,7 @@ void phase_sense(axo_ctx* c) {
                     if (dx * dx + dy * dy + dz * dz > r2) continue;
                     const int x = ci + dx, y = cj + dy, z = ck + dz;
                     if (x < 0 || y < 0 || z < 0 || x >= (int)c->nx || y >= (int)c->ny || z >= (int)c->nz) continue;
-                    const size_t cell = ((size_t)z * c->ny + y) * c->nx + x;
+                    const size_t cell = c->key_of_cell((uint32_t)x, (uint32_t)y, (uint32_t)z);
                     for (uint32_t j = c->cell_start[cell]; j < c->cell_end[cell]; ++j) {
                         const int s = c->A.species[j];
                         n[s] += 1;
@@ -560,6 +574,15 @@ AXO_API int axo_add_source(axo_ctx* c, float x, float y, float z, uint8_t specie
 AXO_API int axo_set_shard(axo_ctx* c, uint32_t rank, uint32_t world) {
     if (!c || world == 0 || rank >= world) return fail(c, EINVAL_, "bad shard");
     c->shard_rank = rank; c->shard_world = world;
+    return OK;
+}
+
+// 0 = linear cell order (default), 1 = bricks of 8 x 4 x 4 cells (reading A-27); only before any particle exists
+AXO_API int axo_set_key_order(axo_ctx* c, int order) {
+    if (!c || (order != 0 && order != 1)) return fail(c, EINVAL_, "bad key order");
+    if (c->stepped || c->A.size() || c->B.size()) return fail(c, ESTATE, "key order must be set before particles exist");
+    c->key_order = order;
+    c->cell_start.clear(); c->cell_end.clear();
     return OK;
 }
 
