@@ -244,6 +244,8 @@ def run_ours(args, w):
 
     def make_sim(D, emission):
         sim_ = axg.Axg(w.grid, D, emission, w.radius, w.speed, w.noise, seed)
+        if args.key_order == "brick":
+            sim_.set_key_order(axg.KEY_BRICK)
         sim_.set_binning(bin_req)
         if world > 1:
             sim_.set_shard(rank, world)   # every rank pre-runs its own shard: particle sets of sources never interact
@@ -418,7 +420,7 @@ def run_ours(args, w):
                            (2 * 17 + 20) * n_end / 1e6),
                        "parallelism": "shard-by-source x%d + int all-reduce" % world if world > 1 else "1 GPU",
                        "prerun": "coarse-time x%d + 100 relax steps" % args.coarse, "steering": args.steering,
-                       "sensing": args.sensing},
+                       "sensing": args.sensing, "key_order": args.key_order},
             "clocks": clock_rec, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "cpu_baseline": cpu,
             "cones": {k: cnt[k] for k in ("active", "arrived", "exited")},
         }
@@ -441,6 +443,8 @@ def main():
     ap.add_argument("--binning", default="auto", choices=("auto", "radix", "count"))
     ap.add_argument("--steering", default="vector", choices=("vector", "snr"),
                     help="P4 rule: north_star's vector addition, or the paper's fixed turn by the sign of N(SNR, 1)")
+    ap.add_argument("--key-order", default="linear", choices=("linear", "brick"),
+                    help="cell key: north_star's linear id, or bricks of 8 x 4 x 4 cells (axg_set_key_order)")
     ap.add_argument("--sensing", default="cell", choices=("cell", "particle", "weighted"),
                     help="P3 rule: north_star's per-cell sums, or the per-particle rule of the paper's section 5.3")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -195,6 +195,20 @@ int axg_set_binning(axg_ctx* ctx, int mode);
 enum { AXG_STEER_VECTOR = 0, AXG_STEER_SNR = 1 };
 int axg_set_steering(axg_ctx* ctx, int mode, float gain, float turn);
 
+/* Cell order = what the cell key of P2a is ("a Z-order curve ... potential
+ * optimization"; reading A-27).
+ *  AXG_KEY_LINEAR (default)  north_star's key: (z * ny + y) * nx + x.
+ *  AXG_KEY_BRICK   bricks of 8 x 4 x 4 cells; bricks in linear order (x fastest), the cells of a brick in linear order:
+ *                  key = (((z/4) * ceil(ny/4) + y/4) * ceil(nx/8) + x/8) * 128 + (z%4) * 32 + (y%4) * 8 + x%8.
+ *                  A particle that moves one cell stays inside, or next to, 512 contiguous bytes of the per-cell
+ *                  arrays.  The key space is the grid padded to whole bricks: AXG_CELL_START / AXG_CELL_END then have
+ *                  ceil(nx/8) * ceil(ny/4) * ceil(nz/4) * 128 entries, indexed by key; AXG_KEYS_SORTED, AXG_PERM and the
+ *                  order of the AXG_PART_* rows follow this key.  Trajectories, cones and all sums are unchanged.
+ * Only directly after axg_create (before neurons, sources or particles exist): AXG_ESTATE otherwise.
+ * AXG_EINVAL: bad value, or a padded key space of 2^32 or more.                                             */
+enum { AXG_KEY_LINEAR = 0, AXG_KEY_BRICK = 1 };
+int axg_set_key_order(axg_ctx* ctx, int order);
+
 /* Sensing rule of P3 (section 5.3: "each individual particle that the axon's
  * growth cone detects would influence the axon's path"; reading A-26).
  *  AXG_SENSE_CELL (default)  north_star's rule: counts and first moments over the CELLS of the index-space ball.

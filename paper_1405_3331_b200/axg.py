@@ -30,6 +30,7 @@ KERNEL_NAMES = ("clear", "diffuse", "emit", "sort", "reorder", "sense", "advance
 BIN_AUTO, BIN_RADIX, BIN_COUNT = 0, 1, 2
 STEER_VECTOR, STEER_SNR = 0, 1
 SENSE_CELL, SENSE_PARTICLE, SENSE_PARTICLE_WEIGHTED = 0, 1, 2
+KEY_LINEAR, KEY_BRICK = 0, 1
 AUTO_COUNT_MAX_CELLS = 1 << 31   # include/axg.h AXG_AUTO_COUNT_MAX_CELLS
 EXPORTS = (
     "axg_create", "axg_place_neurons", "axg_add_source", "axg_step", "axg_read_state", "axg_destroy",
@@ -38,6 +39,7 @@ EXPORTS = (
     "axg_kernel_times", "axg_check_capacity", "axg_enqueue_phase", "axg_sync", "axg_set_binning",
     "axg_set_steering",
     "axg_set_sensing",
+    "axg_set_key_order",
 )
 
 _ALLOC_T = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p)
@@ -90,6 +92,7 @@ def lib(build=True):
     L.axg_set_binning.argtypes = [vp, C.c_int]
     L.axg_set_steering.argtypes = [vp, C.c_int, C.c_float, C.c_float]
     L.axg_set_sensing.argtypes = [vp, C.c_int]
+    L.axg_set_key_order.argtypes = [vp, C.c_int]
     L.axg_load_particles.argtypes = [vp, vp, vp, vp, vp, vp, u64, u32, u32]
     L.axg_load_cones.argtypes = [vp, vp, vp, vp, vp, u32]
     L.axg_read_state.argtypes = [vp, u32, vp, sz, C.POINTER(sz)]
@@ -188,6 +191,9 @@ class Axg:
 
     def set_binning(self, mode):
         self._chk(self._L.axg_set_binning(self._h, int(mode)))
+
+    def set_key_order(self, order):
+        self._chk(self._L.axg_set_key_order(self._h, int(order)))
 
     def set_sensing(self, mode):
         self._chk(self._L.axg_set_sensing(self._h, int(mode)))

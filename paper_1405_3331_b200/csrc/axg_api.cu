@@ -91,7 +91,13 @@ struct axg_ctx {
     float ktimes[AXG_KERNEL_COUNT] = {0};
     std::vector<cudaEvent_t> prof_events;
 
-    size_t cells() const { return (size_t)grid.nx * grid.ny * grid.nz; }
+    int key_order = AXG_KEY_LINEAR;  // axg_set_key_order: AXG_KEY_BRICK pads the key space to whole 8 x 4 x 4 bricks
+    size_t nbx() const { return (grid.nx + 7) / 8; }
+    size_t nby() const { return (grid.ny + 3) / 4; }
+    size_t cells() const {  // size of the key space
+        if (key_order == AXG_KEY_LINEAR) return (size_t)grid.nx * grid.ny * grid.nz;
+        return nbx() * nby() * ((grid.nz + 3) / 4) * 128;
+    }
     // cell arrays are padded to whole scan tiles so that 128-bit accesses of the last tile stay inside
     size_t cells_padded() const { return ((cells() + 1 + AXG_SCAN_TILE - 1) / AXG_SCAN_TILE + 1) * AXG_SCAN_TILE; }
     // look-back words of k_cell_scan (one per tile) / block sums of k_cell_scan2 (one per block, at most 148 x 2)
@@ -181,6 +187,7 @@ int alloc_fixed(axg_ctx* c) {
     P.dev = (AxgDev*)c->d_dev;
     P.cell_lo = (uint32_t*)c->d_cell_lo;
     P.nx = c->grid.nx; P.ny = c->grid.ny; P.nz = c->grid.nz; P.cells = (uint32_t)c->cells();
+    P.key_order = c->key_order; P.nbx = (uint32_t)c->nbx(); P.nby = (uint32_t)c->nby();
     P.fnx = (float)c->grid.nx; P.fny = (float)c->grid.ny; P.fnz = (float)c->grid.nz;
     P.sigma = (float)std::sqrt(2.0 * (double)c->D);  // O0
     P.seed_lo = (uint32_t)(c->seed & 0xffffffffull);
@@ -677,6 +684,16 @@ AXG_API int axg_set_steering(axg_ctx* c, int mode, float gain, float turn) {
     c->P.snr_gain = gain;
     c->P.cos_turn = (float)std::cos((double)turn);
     c->P.sin_turn = (float)std::sin((double)turn);
+    return AXG_OK;
+}
+
+AXG_API int axg_set_key_order(axg_ctx* c, int order) {
+    if (!c || (order != AXG_KEY_LINEAR && order != AXG_KEY_BRICK)) return fail(c, AXG_EINVAL, "bad key order");
+    if (order == c->key_order) return AXG_OK;
+    if (c->d_dev) return fail(c, AXG_ESTATE, "the key order must be set directly after axg_create");
+    const size_t brick_cells = c->nbx() * c->nby() * ((c->grid.nz + 3) / 4) * 128;
+    if (order == AXG_KEY_BRICK && brick_cells >= (1ull << 32)) return fail(c, AXG_EINVAL, "padded key space >= 2^32");
+    c->key_order = order;
     return AXG_OK;
 }
 

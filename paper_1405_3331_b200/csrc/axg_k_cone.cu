@@ -30,7 +30,7 @@ __global__ void __launch_bounds__(256) k_sense(const AxgParams p) {
                       dz = (int)(int8_t)((o >> 16) & 0xff);
             const int x = ci + dx, y = cj + dy, z = ck + dz;
             if (x < 0 || y < 0 || z < 0 || x >= (int)p.nx || y >= (int)p.ny || z >= (int)p.nz) continue;
-            const uint32_t cell = ((uint32_t)z * p.ny + (uint32_t)y) * p.nx + (uint32_t)x;
+            const uint32_t cell = axg_key_of_cell(p, (uint32_t)x, (uint32_t)y, (uint32_t)z);
             const uint32_t a = __ldg(cell_lo + cell), b = __ldg(cell_lo + cell + 1);
             if (p.single_species >= 0) {
                 const int cnt = (int)(b - a);
@@ -117,7 +117,10 @@ __global__ void __launch_bounds__(256) k_sense_particles(const AxgParams p) {
         for (int s = 0; s < AXG_MAX_SPECIES_D; ++s)
 #pragma unroll
             for (int a = 0; a < 4; ++a) acc[s][a] = 0;
-        for (int r0 = 0; r0 < n_rows; r0 += 32) {
+        // bricked cell order: the x range of a row crosses at most max_seg bricks, one contiguous run in each
+        const int max_seg = p.key_order ? ((2 * (int)ceilf(Rm) + 8) >> 3) + 1 : 1;
+        for (int r0 = 0; r0 < n_rows; r0 += 32)
+        for (int seg = 0; seg < max_seg; ++seg) {
             const int r = r0 + lane;
             uint32_t a = 0, b = 0;
             if (r < n_rows) {
@@ -128,11 +131,15 @@ __global__ void __launch_bounds__(256) k_sense_particles(const AxgParams p) {
                 const float left = Rm * Rm - (ey * ey + ez * ez);
                 if (left >= 0.0f) {
                     const float hw = sqrtf(left) * 1.00001f + 1e-5f;
-                    const int x0 = max(0, (int)floorf(qx - hw)), x1 = min((int)p.nx - 1, (int)floorf(qx + hw));
+                    int x0 = max(0, (int)floorf(qx - hw)), x1 = min((int)p.nx - 1, (int)floorf(qx + hw));
+                    if (p.key_order) {  // the seg-th brick of the range
+                        const int bx = (x0 >> 3) + seg;
+                        x0 = max(x0, bx << 3);
+                        x1 = min(x1, (bx << 3) + 7);
+                    }
                     if (x1 >= x0) {
-                        const uint32_t row = ((uint32_t)z * p.ny + (uint32_t)y) * p.nx;
-                        a = __ldg(cell_lo + row + (uint32_t)x0);
-                        b = __ldg(cell_lo + row + (uint32_t)x1 + 1u);
+                        a = __ldg(cell_lo + axg_key_of_cell(p, (uint32_t)x0, (uint32_t)y, (uint32_t)z));
+                        b = __ldg(cell_lo + axg_key_of_cell(p, (uint32_t)x1, (uint32_t)y, (uint32_t)z) + 1u);
                     }
                 }
             }

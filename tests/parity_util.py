@@ -6,10 +6,13 @@ from paper_1405_3331_b200 import workloads as W
 
 RTOL, ATOL = 1e-5, 1e-6   # BASELINE.json north_star: single-step fp32 positions, gradients, headings
 BINNING = None            # axg.BIN_RADIX / axg.BIN_COUNT: set by the parametrised fixture of the GPU tests
+KEY_ORDER = 0             # 1: both sides use the bricked cell order (include/axg.h axg_set_key_order)
 
 
 def new_axg(axg_mod, *args):
     g = axg_mod.Axg(*args)
+    if KEY_ORDER:
+        g.set_key_order(KEY_ORDER)
     if BINNING is not None:
         g.set_binning(BINNING)
     return g
@@ -19,6 +22,8 @@ def make_pair(w, axg_mod, place=True):
     """The same workload applied to a CUDA context and an oracle context."""
     g = new_axg(axg_mod, w.grid, w.D, w.emission, w.radius, w.speed, w.noise, w.seed)
     o = axo.Oracle(w.grid, w.D, w.emission, w.radius, w.speed, w.noise, w.seed)
+    if KEY_ORDER:
+        o.set_key_order(KEY_ORDER)
     W.apply(g, w, place=place)
     W.apply(o, w, place=place)
     return g, o

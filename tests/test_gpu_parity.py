@@ -335,3 +335,54 @@ def test_particle_sensing_against_the_closed_form(axg, mode, coef):
         assert abs(M[1] - expect[1]) < 0.09 * abs(expect[1]), (R, M, expect)
         assert abs(M[2]) < 0.05 * abs(expect[0]), (R, M, expect)
         np.testing.assert_allclose(cnt, rho0 * (1 + (c.astype(np.float64) - 8.0) @ k) * 4 * np.pi / 3 * R ** 3, rtol=0.03)
+
+
+@pytest.fixture
+def brick_order():
+    pu.KEY_ORDER = 1
+    yield
+    pu.KEY_ORDER = 0
+
+
+@pytest.mark.parametrize("sensing", [None, 1])
+def test_chain_brick_order(axg, brick_order, sensing):
+    """SURVEY.md §8(f) NEXT-4 (reading A-27): the bricked cell order on both sides.  Grids that are whole bricks
+    (24 x 20 x 16), ragged ones (40 x 33 x 21: padded key space 40 x 36 x 24; 6 x 5 x 4: one partial brick) and a 3-pass key
+    (128 x 128 x 64); keys, permutation, cellStart / cellEnd (indexed by brick key), sums bit-exact as under the linear order."""
+    _chain(axg, W.small(seed=7), n=50_037, seed=11, steps=3, sensing=sensing)
+    _chain(axg, W.small(seed=8, two_species=False, grid=(40, 33, 21), n_cones=200), n=30_011, seed=12, steps=2,
+           n_species=1, sensing=sensing)
+    w = W.small(seed=17, grid=(6, 5, 4), n_cones=9)
+    w.D = 8.0
+    _chain(axg, w, n=30_011, seed=19, steps=2, sensing=sensing)
+    w = W.small(seed=9, grid=(128, 128, 64), n_cones=300, n_sources=5, radius=3.0)
+    w.D = 1.0
+    w.max_particles = 1 << 18
+    _chain(axg, w, n=200_003, seed=13, steps=2, sensing=sensing)
+
+
+def test_brick_order_changes_only_the_order(axg):
+    """30 whole steps under either cell order: the same particles (by id, bit for bit), the same cones and polylines; and
+    the order can no longer be changed once the context holds anything."""
+    w = W.small(seed=41, grid=(40, 33, 21), n_cones=300, n_sources=4, rate=300)
+    w.max_particles = 1 << 18
+    out = []
+    for order in (axg.KEY_LINEAR, axg.KEY_BRICK):
+        g = axg.Axg(w.grid, w.D, w.emission, w.radius, w.speed, w.noise, w.seed)
+        g.set_key_order(order)
+        if pu.BINNING is not None:
+            g.set_binning(pu.BINNING)
+        W.apply(g, w)
+        x, y, z, sp, ids = W.random_particles(43, 120_007, w.grid, n_species=2)
+        g.load_particles(x, y, z, sp, ids, next_id=len(ids), step=0)
+        g.step(30)
+        with pytest.raises(axg.AxgError):
+            g.set_key_order(1 - order)
+        srt = np.argsort(g.read_state("PART_ID"))
+        out.append([g.read_state("PART_" + k)[srt] for k in ("ID", "X", "Y", "Z", "SPECIES")] +
+                   [g.read_state(k) for k in ("CONE_POS", "CONE_HEADING", "CONE_STATE", "POLYLINE", "CONE_MOMENT")])
+        ks = g.read_state("KEYS_SORTED")
+        assert (np.diff(ks.astype(np.int64)) >= 0).all()
+        g.close()
+    for a, b in zip(*out):
+        assert np.array_equal(a.view(np.uint8), b.view(np.uint8))
