@@ -130,3 +130,54 @@ def test_particle_sensing_on_sampled_cones(c3, mode):
     assert np.array_equal(gm, o.read_state("CONE_MOMENT").reshape(-1, 12)[pick])
     assert gc.sum() > 0
     o.close()
+
+
+def test_brick_order_at_full_size():
+    """C3 under the bricked cell order (reading A-27), the configuration `bench.py --key-order brick` times:
+    properties that hold at any size, the key restated in numpy, sampled cells, and sampled cones recomputed all pairs."""
+    from paper_1405_3331_b200 import axg as m
+    m.lib()
+    w = W.c3()
+    w.max_segments = 32
+
+    def make(D, e):
+        s = m.Axg(w.grid, D, e, w.radius, w.speed, w.noise, w.seed)
+        s.set_key_order(m.KEY_BRICK)
+        return s
+
+    sim = W.prerun(make, w, coarse=16, relax=20)
+    try:
+        sim.step(3)
+        n = sim.counters()["n_live"]
+        assert n > 5_000_000
+        a = _arrays(sim)
+        nx, ny, nz = w.grid
+        ix, iy, iz = a["X"].astype(np.int64), a["Y"].astype(np.int64), a["Z"].astype(np.int64)
+        key = ((iz // 4 * (ny // 4) + iy // 4) * (nx // 8) + ix // 8) * 128 + iz % 4 * 32 + iy % 4 * 8 + ix % 8
+        ks = sim.read_state("KEYS_SORTED").astype(np.int64)
+        assert np.array_equal(key, ks) and (np.diff(ks) >= 0).all()
+        perm = sim.read_state("PERM")
+        assert len(perm) == n and np.array_equal(np.sort(perm), np.arange(n, dtype=np.uint32))
+        same = ks[1:] == ks[:-1]
+        assert (perm[1:][same] > perm[:-1][same]).all()
+        assert len(np.unique(a["ID"])) == n
+        cs, ce = sim.read_state("CELL_START").astype(np.int64), sim.read_state("CELL_END").astype(np.int64)
+        assert len(cs) == nx * ny * nz and (ce - cs).sum() == n
+        rng = np.random.default_rng(6)
+        for cell in np.concatenate([rng.integers(0, len(cs), 200), rng.choice(ks, 200)]):
+            lo, hi = np.searchsorted(ks, cell), np.searchsorted(ks, cell, side="right")
+            assert (cs[cell], ce[cell]) == ((lo, hi) if hi > lo else (0, 0))
+        sim.step_phase(m.PHASE_SENSE)
+        counts = sim.read_state("CONE_COUNTS").reshape(-1, 4)
+        moment = sim.read_state("CONE_MOMENT").reshape(-1, 4, 3)
+        pos = sim.read_state("CONE_POS").reshape(-1, 3)
+        active = np.flatnonzero(sim.read_state("CONE_STATE") == 0)
+        for cone in rng.choice(active, min(12, len(active)), replace=False):
+            d = np.stack([ix - int(pos[cone, 0]), iy - int(pos[cone, 1]), iz - int(pos[cone, 2])], 1)
+            near = (d * d).sum(1) <= int(w.radius * w.radius)
+            for s in range(4):
+                sel = near & (a["SPECIES"] == s)
+                assert counts[cone, s] == sel.sum()
+                assert np.array_equal(moment[cone, s], d[sel].sum(0) if sel.any() else np.zeros(3, np.int64))
+    finally:
+        sim.close()
