@@ -78,6 +78,8 @@ enum {
     AXG_PART_ID = 5,      /* u32[n_live]                                                                */
     AXG_KEYS_SORTED = 6,  /* u32[n_live]                                                                */
     AXG_PERM = 7,         /* u32[n_live]  sorted j -> pre-sort index                                    */
+                          /* (6, 7: those of the last completed P2; under count binning they are not stored on the path
+                           *  but derived here, on read, from the intact inputs of that P2; undefined between a P1 and its P2) */
     AXG_CELL_START = 8,   /* u32[cells]   first sorted j of the cell, 0 if empty                        */
     AXG_CELL_END = 9,     /* u32[cells]   one past the last sorted j, 0 if empty                        */
     AXG_CONE_POS = 10,    /* f32[C*3] AoS                                                               */
