@@ -46,6 +46,8 @@ TRAFFIC_NCU = {   # (workload, kernel) -> bytes per launch; profiles/r01_summary
     ("C3", "k_place"): 248.8e6, ("C3", "k_cell_scan2"): 172.6e6, ("C3", "k_sort_pass"): 203.7e6,
     ("C3", "k_reorder"): 740.8e6,
 }
+# the same capture summed over the kernels of one step (count binning: P1 + scan + place + settle + sense + advance)
+STEP_TRAFFIC_NCU = {("C3", "count"): 1832.0e6}
 
 
 def log(*a):
@@ -88,63 +90,126 @@ def bytes_model(w, n_live, n_active_cones, n_stencil, count_mode):
              "settle": 45.0 * n_live,              # slot 4 + record 16 + cell_lo 8 + SoA 17 (keys / perm: derived on read)
              "sense": sense}
         launches = {"diffuse": 1, "scan": 1, "place": 1, "settle": 1, "sense": 1}
+        # SURVEY.md §8(d) bytes of the phases these kernels stand for: K1 38; sort (12 + 16 (passes - 1)) split over scan
+        # and place (which together replace the digit passes); reorder + cell ranges 42 B + 8 B per cell
+        sort_b = (12.0 + 16.0 * (passes - 1)) * n_live
+        survey = {"diffuse": 38.0 * n_live, "scan": 8.0 * w.cells, "place": sort_b, "settle": 42.0 * n_live, "sense": sense}
     else:
         k = {"diffuse": 38.0 * n_live,
              "sort": (12.0 + 16.0 * (passes - 1)) * n_live,   # pass 0: 4 read + 8 write; later passes 8 + 8
              "reorder": 42.0 * n_live + 4.0 * w.cells,        # perm 4 + key 4 + gather 17 + write 17; 4 B / cell
              "sense": sense}
         launches = {"diffuse": 1, "sort": passes, "reorder": 1, "sense": 1}
-    return step, k, launches
+        survey = {"diffuse": 38.0 * n_live, "sort": (12.0 + 16.0 * (passes - 1)) * n_live,
+                  "reorder": 42.0 * n_live + 8.0 * w.cells, "sense": sense}
+    return step, k, launches, survey
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md clocks line)."""
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
-         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
-         "clocks_event_reasons.sw_power_cap")
+    """SM clock and throttle reasons sampled DURING the run (B200_PROFILING.md clocks line): a thread that polls NVML
+    every millisecond from before the warm-up to after the last measured phase (ctypes calls release the GIL, so it
+    runs while axg_step blocks).  `mark()` brackets the timed region; the record reports the samples that fell inside
+    it and, separately, all samples under load.  Falls back to an `nvidia-smi -lms` subprocess without pynvml."""
+
+    REASONS = ((0x8, "hw_slowdown"), (0x40, "hw_thermal_slowdown"), (0x20, "sw_thermal_slowdown"), (0x4, "sw_power_cap"))
 
     def __init__(self, index):
-        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
-        self.p = None
+        import threading
+        self.samples = []      # (t, sm_mhz, reasons bitmask, power_w)
+        self.t0 = self.t1 = None
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thread = None
         try:
-            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
-                                       "--format=csv,noheader,nounits", "-lms", "50"], stdout=self.f,
-                                      stderr=subprocess.DEVNULL)
+            import pynvml
+            pynvml.nvmlInit()
+            idx = index
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            if vis:
+                try:
+                    idx = int(vis.split(",")[index])
+                except (ValueError, IndexError):
+                    idx = index
+            h = pynvml.nvmlDeviceGetHandleByIndex(idx)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+            reasons = getattr(pynvml, "nvmlDeviceGetCurrentClocksEventReasons", None) or \
+                pynvml.nvmlDeviceGetCurrentClocksThrottleReasons
+
+            def poll():
+                while not self._stop.is_set():
+                    try:
+                        self.samples.append((time.time(), float(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM)),
+                                             int(reasons(h)), pynvml.nvmlDeviceGetPowerUsage(h) / 1000.0))
+                    except Exception:
+                        pass
+                    self._stop.wait(0.001)
+            self._thread = threading.Thread(target=poll, daemon=True)
+            self._thread.start()
+        except Exception as e:    # no NVML binding: the recipe's nvidia-smi line, 20 ms period
+            log("[bench] pynvml unavailable (%s): nvidia-smi sampler" % e)
+            self._smi(index)
+
+    def _smi(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=timestamp,clocks.sm,clocks.max.sm,"
+                                       "power.draw,clocks_event_reasons.hw_slowdown,"
+                                       "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+                                       "clocks_event_reasons.sw_power_cap", "--format=csv,noheader,nounits", "-lms", "20"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
         except Exception:
             self.p = None
 
+    def mark(self, begin):
+        if begin:
+            self.t0 = time.time()
+        else:
+            self.t1 = time.time()
+
     def stop(self):
-        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
-        if self.p is None:
-            return out
-        self.p.terminate()
-        try:
-            self.p.wait(timeout=5)
-        except Exception:
-            self.p.kill()
-        self.f.flush()
-        self.f.seek(0)
-        sm, mx, pw, reasons = [], [], [], set()
-        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
-        for line in self.f:
-            c = [x.strip() for x in line.split(",")]
-            if len(c) < 7:
-                continue
+        import datetime
+        self._stop.set()
+        if self._thread is not None:
+            self._thread.join(timeout=2)
+        elif getattr(self, "p", None) is not None:
+            self.p.terminate()
             try:
-                sm.append(float(c[0])); mx.append(float(c[1])); pw.append(float(c[2]))
-            except ValueError:
-                continue
-            for nm, v in zip(names, c[3:7]):
-                if v == "Active":
-                    reasons.add(nm)
-        self.f.close()
-        try:
-            os.unlink(self.f.name)
-        except OSError:
-            pass
-        if sm:
-            out = {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
-                   "samples": len(sm), "power_w_max": float(max(pw))}
+                self.p.wait(timeout=5)
+            except Exception:
+                self.p.kill()
+            self.f.flush()
+            self.f.seek(0)
+            for line in self.f:
+                c = [x.strip() for x in line.split(",")]
+                if len(c) < 8:
+                    continue
+                try:
+                    t = datetime.datetime.strptime(c[0], "%Y/%m/%d %H:%M:%S.%f").timestamp()
+                    mask = sum(bit for (bit, _), v in zip(self.REASONS, c[4:8]) if v == "Active")
+                    self.samples.append((t, float(c[1]), mask, float(c[3])))
+                    self.max_mhz = float(c[2])
+                except ValueError:
+                    continue
+            self.f.close()
+            try:
+                os.unlink(self.f.name)
+            except OSError:
+                pass
+        out = {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0}
+        if not self.samples:
+            return out
+        inside = [x for x in self.samples if self.t0 is not None and self.t1 is not None and self.t0 <= x[0] <= self.t1]
+        busy = [x for x in self.samples if x[3] > 0.5 * max(y[3] for y in self.samples)] or self.samples
+        use = inside or busy
+        mask = 0
+        for x in use:
+            mask |= x[2]
+        out.update({"sm_mhz": float(np.median([x[1] for x in use])), "samples": len(inside),
+                    "samples_under_load": len(busy), "sm_mhz_under_load": float(np.median([x[1] for x in busy])),
+                    "reasons": [nm for bit, nm in self.REASONS if mask & bit],
+                    "power_w_max": float(max(x[3] for x in self.samples)),
+                    "how": "NVML polled every ms in a thread; sm_mhz / reasons = the samples inside the timed region "
+                           "(all samples under load if none fell inside)"})
         return out
 
 
@@ -239,13 +304,11 @@ def run_ours(args, w):
     seed = w.seed
 
     bin_req = {"auto": axg.BIN_AUTO, "radix": axg.BIN_RADIX, "count": axg.BIN_COUNT}[args.binning]
-    count_mode = bin_req == axg.BIN_COUNT or (bin_req == axg.BIN_AUTO and w.cells <= axg.AUTO_COUNT_MAX_CELLS and
-                                              w.cells <= 4 * (w.max_particles or 1 << 20))
 
     def make_sim(D, emission):
         sim_ = axg.Axg(w.grid, D, emission, w.radius, w.speed, w.noise, seed)
-        if args.key_order == "brick":
-            sim_.set_key_order(axg.KEY_BRICK)
+        if args.key_order != "linear":
+            sim_.set_key_order(axg.KEY_BRICK if args.key_order == "brick" else axg.KEY_MORTON)
         sim_.set_binning(bin_req)
         if world > 1:
             sim_.set_shard(rank, world)   # every rank pre-runs its own shard: particle sets of sources never interact
@@ -257,10 +320,11 @@ def run_ours(args, w):
         sim.set_steering(axg.STEER_SNR, 8.0, np.pi / 30)
     if args.sensing != "cell":
         sim.set_sensing(axg.SENSE_PARTICLE if args.sensing == "particle" else axg.SENSE_PARTICLE_WEIGHTED)
-    if world > 1:
+    if world > 1 or args.force_sharded_loop:
         step = sharded.ShardedStepper(sim, rank, world, sharded.nccl_exchange).step
     else:
         step = sim.step
+    count_mode = sim.get_binning() == axg.BIN_COUNT     # what AXG_BIN_AUTO resolved to, asked of the library
     c0 = sim.counters()
     log("[bench] rank %d: %s steady state in %.1f s: n_live=%d" % (rank, w.name, time.time() - t0, c0["n_live"]))
 
@@ -291,11 +355,13 @@ def run_ours(args, w):
         return float(v)
 
     # ---- warm-up, then the timed region: exactly K steps, inputs resident in HBM ------------------------------
+    clocks = ClockSampler(local)    # from before the warm-up to after the last measured phase
     step(Wm)
     n_start = sim.counters()["n_live"]
-    clocks = ClockSampler(local)
     torch.cuda.profiler.start()     # `ncu --profile-from-start off` captures the timed region only
+    clocks.mark(True)
     ms = timed(lambda: step(K))
+    clocks.mark(False)
     torch.cuda.profiler.stop()
     st = sim.last_step_stats()
     psteps = total(st["particle_steps"])
@@ -313,6 +379,24 @@ def run_ours(args, w):
         st2 = sim.last_step_stats()
         n_avg = st2["particle_steps"] / K
         active = sim.counters()["active"]
+    # ---- the path north_star spells out (onesweep radix passes + reorder), timed on the same state, same K ---------
+    radix_rec = None
+    if world == 1 and count_mode and not args.no_radix_record:
+        sim.set_binning(axg.BIN_RADIX)
+        step(Wm)
+        ms_r = timed(lambda: step(K))
+        ps_r = sim.last_step_stats()["particle_steps"]
+        sim.profile_next_step(True)
+        step(K)
+        kt_r = sim.kernel_times()
+        sort_ms = kt_r["sort"] / K
+        radix_rec = {"ms_per_step": ms_r / K, "particle_steps_per_s": ps_r / (ms_r * 1e-3),
+                     "sort_ms_per_step": sort_ms, "passes": key_passes(w.cells),
+                     "sort_keys_per_s": (sim.last_step_stats()["particle_steps"] / K) / max(sort_ms * 1e-3, 1e-12),
+                     "kernels_ms_per_step": {k: round(v / K, 5) for k, v in kt_r.items() if v > 0},
+                     "what": "axg_set_binning(AXG_BIN_RADIX): k_diffuse (chained compaction), one k_sort_pass per 8-bit "
+                             "digit, k_reorder; same state, same K, bit-identical results"}
+        sim.set_binning(bin_req)
     clock_rec = clocks.stop()
 
     # ---- roofline of the dominant kernel: algorithmic bytes per launch / CUDA-event time -------
@@ -323,28 +407,54 @@ def run_ours(args, w):
                     if dx * dx + dy * dy + dz * dz <= r2)
     extra = {}
     if ktimes is not None:
-        step_bytes, bm, launches_of = bytes_model(w, n_avg, active, n_stencil, count_mode)
+        step_bytes, bm, launches_of, survey = bytes_model(w, n_avg, active, n_stencil, count_mode)
         per_step_ms = {k: v / K for k, v in ktimes.items()}
         kernel_name = {"diffuse": "k_diffuse_chunked" if count_mode else "k_diffuse", "sort": "k_sort_pass", "reorder": "k_reorder", "sense": "k_sense",
                        "scan": "k_cell_scan2", "place": "k_place", "settle": "k_settle"}
         dom = max(bm.keys(), key=lambda k: per_step_ms[k])
         per_launch_ms = per_step_ms[dom] / launches_of[dom]
-        per_launch_bytes = bm[dom] / launches_of[dom]
+        own_bytes = bm[dom] / launches_of[dom]
+        # `achieved` / `frac` follow SURVEY.md §8(d): the METHOD's bytes for this phase (P1: 17 read + 17 written + 4 key
+        # = 38 B per particle, whatever this kernel's own layout moves); `frac_own_bytes` uses what the kernel itself
+        # must move (P1 of count binning writes a 16 B record + an 8 B {key, arrival rank} word and issues
+        # one 4 B counting atomic = 45 B)
+        per_launch_bytes = survey[dom] / launches_of[dom]
         achieved = per_launch_bytes / (per_launch_ms * 1e-3) / 1e9
         roof = {"bound": "hbm", "kernel": kernel_name[dom], "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": TRAFFIC_NCU.get((w.name, kernel_name[dom])),
                 "peak_source": peak_src, "launches_per_step": launches_of[dom],
                 "algorithmic_bytes_per_launch": per_launch_bytes, "ms_per_launch": per_launch_ms,
+                "bytes_convention": "SURVEY.md 8(d) per-phase bytes of the method",
+                "frac_own_bytes": own_bytes / (per_launch_ms * 1e-3) / 1e9 / peak, "own_bytes_per_launch": own_bytes,
                 "share_of_step": per_step_ms[dom] / max(sum(per_step_ms.values()), 1e-12)}
         step_ms = ms / K
         step_gbs = step_bytes / (step_ms * 1e-3) / 1e9
-        extra["roofline_step"] = {"achieved": step_gbs, "unit": "GB/s", "frac_of_measured_copy": step_gbs / peak,
-                                  "frac_of_nominal_8TBs": step_gbs / NOMINAL_GBS,
-                                  "algorithmic_bytes_per_particle": step_bytes / max(n_avg, 1)}
+        moved = sum(bm.values())     # what the kernels of the benchmarked binning mode must move themselves
+        dram = STEP_TRAFFIC_NCU.get((w.name, "count" if count_mode else "radix"))
+        extra["roofline_step"] = {
+            "achieved": step_gbs, "unit": "GB/s", "frac_of_measured_copy": step_gbs / peak,
+            "frac_of_nominal_8TBs": step_gbs / NOMINAL_GBS,
+            "algorithmic_bytes_per_particle": step_bytes / max(n_avg, 1),
+            "bytes_convention": "SURVEY.md 8(d): bytes of the METHOD (K1 38 + 3-pass sort 44 + reorder 42 B per particle "
+                                "+ 8 B per cell + cones), whatever the binning mode moves",
+            "own_bytes_per_particle": moved / max(n_avg, 1),
+            "frac_own_bytes_of_measured_copy": moved / (step_ms * 1e-3) / 1e9 / peak,
+            "frac_own_bytes_of_nominal_8TBs": moved / (step_ms * 1e-3) / 1e9 / NOMINAL_GBS,
+            "dram_bytes_per_step_ncu": dram,
+            "frac_dram_of_measured_copy": None if dram is None else dram / (step_ms * 1e-3) / 1e9 / peak,
+            "frac_dram_of_nominal_8TBs": None if dram is None else dram / (step_ms * 1e-3) / 1e9 / NOMINAL_GBS,
+            "dram_note": "dram__bytes_read+write summed over one step's kernels in the committed ncu capture (profiles/); "
+                         "below the algorithmic bytes where the 126 MB L2 holds the per-cell arrays"}
+        extra["materialised"] = (
+            "count binning: the sorted SoA and the prefix array cell_lo are written every step; KEYS_SORTED / PERM and "
+            "cellStart / cellEnd are derived on read (axg_read_state), bit-identical to the radix path that stores them"
+            if count_mode else "radix binning: sorted keys, permutation, sorted SoA and cell_lo are written every step")
         extra["kernels_ms_per_step"] = {k: round(v, 5) for k, v in per_step_ms.items() if v > 0}
         extra["kernels_gbs"] = {k: bm[k] / (per_step_ms[k] * 1e-3) / 1e9 for k in bm if per_step_ms[k] > 0}
         extra["cone_steps_per_s"] = active / (step_ms * 1e-3)
         extra["binning"] = "count" if count_mode else "radix"
+        if radix_rec:
+            extra["radix"] = radix_rec
 
     # ---- e2e: the same job through the C-ABI with HOST buffers; every host<->device copy inside the timed region --
     # upload of the particle SoA + cone state from pinned host memory, then e2e_steps x [axg_step(1), read back cone
@@ -367,7 +477,7 @@ def run_ours(args, w):
         sim.read_state("CONE_STATE", out=cone_state)
         sim.read_state("POLY_LEN", out=poly_len)
     out_cols = [pinned(n_now + (e2e_steps + 1) * w.emitted_per_step + 64, d) for d in dts]
-    counters_host = pinned(8, np.uint64)
+    counters_host = pinned(16, np.uint64)
     h2d = d2h = 0
     e2e_psteps = 0
 
@@ -443,11 +553,15 @@ def main():
     ap.add_argument("--binning", default="auto", choices=("auto", "radix", "count"))
     ap.add_argument("--steering", default="vector", choices=("vector", "snr"),
                     help="P4 rule: north_star's vector addition, or the paper's fixed turn by the sign of N(SNR, 1)")
-    ap.add_argument("--key-order", default="linear", choices=("linear", "brick"),
-                    help="cell key: north_star's linear id, or bricks of 8 x 4 x 4 cells (axg_set_key_order)")
+    ap.add_argument("--key-order", default="linear", choices=("linear", "brick", "morton"),
+                    help="cell key: north_star's linear id, bricks of 8 x 4 x 4 cells, or the Z-order curve (axg_set_key_order)")
     ap.add_argument("--sensing", default="cell", choices=("cell", "particle", "weighted"),
                     help="P3 rule: north_star's per-cell sums, or the per-particle rule of the paper's section 5.3")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--force-sharded-loop", action="store_true",
+                    help="run the multi-GPU step loop (sharded.ShardedStepper) also at N = 1, to time it against axg_step")
+    ap.add_argument("--no-radix-record", action="store_true",
+                    help="skip the `radix` sub-record (the same K steps under AXG_BIN_RADIX)")
     args = ap.parse_args()
     from paper_1405_3331_b200 import workloads as W
     w = W.BY_NAME[args.workload]()

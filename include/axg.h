@@ -44,7 +44,12 @@ typedef struct axg_grid {
 enum {
     AXG_OK = 0,
     AXG_EINVAL = -1,    /* bad argument (null, NaN, out of the domain, radius not in [1,8], cells >= 2^32 ...)   */
-    AXG_ECAPACITY = -2, /* particle or polyline capacity would overflow (checked on host bounds before launch) */
+    AXG_ECAPACITY = -2, /* particle or polyline capacity would overflow (checked on host bounds before launch); or the
+                           device error word was found set after a synchronisation (only reachable through
+                           axg_enqueue_phase, which checks nothing): the step that hit the capacity dropped its emission
+                           or its append, so the state is UNDEFINED from there on.  The word is cleared when it is
+                           reported, by axg_set_capacity and by axg_load_particles: raise the capacity, reload the
+                           state, go on.                                                                           */
     AXG_ESTATE = -3,    /* call not allowed in this state (neurons placed after the first step)                */
     AXG_ECUDA = -4,     /* CUDA runtime error, or no device                                                    */
     AXG_ESMALL = -5     /* dst_bytes too small; *n_elems holds the element count required                      */
@@ -55,7 +60,7 @@ enum {
 #define AXG_R_CAPTURE 1.0f /* arrival radius in cells (reading A-16) */
 
 /* cone state */
-enum { AXG_CONE_ACTIVE = 0, AXG_CONE_ARRIVED = 1, AXG_CONE_EXITED = 2 };
+enum { AXG_CONE_ACTIVE = 0, AXG_CONE_ARRIVED = 1, AXG_CONE_EXITED = 2, AXG_CONE_CONNECTED = 3 /* axg_set_connect */ };
 
 /* phases for axg_step_phase */
 enum {
@@ -64,13 +69,15 @@ enum {
     AXG_PHASE_SENSE = 4,   /* P3                                                                     */
     AXG_PHASE_ADVANCE = 8, /* P4 + P5                                                                */
     AXG_PHASE_COMMIT = 16, /* step counter t += 1                                                    */
-    AXG_PHASE_ALL = 31
+    AXG_PHASE_ALL = 31,
+    AXG_PHASE_CONNECT = 32 /* connection formation after P5 (axg_set_connect; a no-op while it is off); part of every
+                              whole step of axg_step once enabled, not of AXG_PHASE_ALL                              */
 };
 
 /* fields for axg_read_state.  "sorted order" = the particle array left by P2 (input of the next P1).
  * "pre-sort" = the array written by P1 (survivors in input order, then newborns), input of P2.         */
 enum {
-    AXG_COUNTERS = 0,     /* u64[8]: step, n_live, next_id, emitted, absorbed, active, arrived, exited  */
+    AXG_COUNTERS = 0,     /* u64[9]: step, n_live, next_id, emitted, absorbed, active, arrived, exited, connected */
     AXG_PART_X = 1,       /* f32[n_live]  sorted order                                                  */
     AXG_PART_Y = 2,
     AXG_PART_Z = 3,
@@ -96,7 +103,11 @@ enum {
     AXG_PRE_SPECIES = 21,
     AXG_PRE_ID = 22,
     AXG_PRE_KEY = 23,     /* u32[n_live]  cell key of the pre-sort array                                */
-    AXG_FIELD_COUNT = 24
+    AXG_CONE_TARGET = 24, /* u32[C]  neuron the cone has connected to, 0xffffffff = none (axg_set_connect)      */
+    AXG_GRAPH_VA = 25,    /* u32[C+1] heads of the adjacency lists (axg_build_graph); empty before              */
+    AXG_GRAPH_EA = 26,    /* u32[E]   edges: neighbours of vertex i at Ea[Va[i] .. Va[i+1]), ascending          */
+    AXG_BFS_LEVEL = 27,   /* i32[C]   BFS level from the root of the last axg_bfs, -1 = not reached             */
+    AXG_FIELD_COUNT = 28
 };
 
 /* Create a context on the current CUDA device.
@@ -150,7 +161,10 @@ const char* axg_last_error(const axg_ctx* ctx);
 int axg_set_capacity(axg_ctx* ctx, uint64_t max_particles, uint32_t max_segments);
 
 /* Replace the particle array (taken as the "sorted order" array, i.e. the input of the next P1) and the id /
- * step counters.  No validation of positions beyond n <= capacity.                                       */
+ * step counters, and clear the device error word.  Positions are not validated here (n <= capacity and species < 4
+ * are): P1 absorbs a row that is outside the domain after its move like any other; AXG_PHASE_BIN without
+ * AXG_PHASE_DIFFUSE on a row outside the domain fails with AXG_EINVAL (device error word bit 4; the row is binned into
+ * cell 0, nothing is written out of bounds, the state is undefined).                                        */
 int axg_load_particles(axg_ctx* ctx, const float* x, const float* y, const float* z, const uint8_t* species,
                        const uint32_t* id, uint64_t n, uint32_t next_id, uint32_t step);
 
@@ -183,6 +197,9 @@ int axg_set_shard(axg_ctx* ctx, uint32_t rank, uint32_t world);
 enum { AXG_BIN_AUTO = 0, AXG_BIN_RADIX = 1, AXG_BIN_COUNT = 2 };
 #define AXG_AUTO_COUNT_MAX_CELLS 2147483648u
 int axg_set_binning(axg_ctx* ctx, int mode);
+/* *mode = AXG_BIN_RADIX or AXG_BIN_COUNT: what the requested mode resolves to for the current grid, key order and
+ * capacity (allocates the particle arrays if they do not exist yet).                                         */
+int axg_get_binning(axg_ctx* ctx, int* mode);
 
 /* Steering rule of P4.
  *  AXG_STEER_VECTOR (default)  north_star's rule: heading = normalise(gradient direction + noise x N(0, I)).
@@ -206,9 +223,13 @@ int axg_set_steering(axg_ctx* ctx, int mode, float gain, float turn);
  *                  arrays.  The key space is the grid padded to whole bricks: AXG_CELL_START / AXG_CELL_END then have
  *                  ceil(nx/8) * ceil(ny/4) * ceil(nz/4) * 128 entries, indexed by key; AXG_KEYS_SORTED, AXG_PERM and the
  *                  order of the AXG_PART_* rows follow this key.  Trajectories, cones and all sums are unchanged.
+ *  AXG_KEY_MORTON  the Z-order curve the paper names (reading A-31): bit b of x, of y and of z in turn, b = 0,
+ *                  1, ..., from the least significant key bit up; an axis that needs fewer bits than the others drops out
+ *                  of the rotation once its bits are used.  Key space = the grid padded to powers of two; indexing of
+ *                  AXG_CELL_START / AXG_CELL_END etc. as under AXG_KEY_BRICK.
  * Only directly after axg_create (before neurons, sources or particles exist): AXG_ESTATE otherwise.
  * AXG_EINVAL: bad value, or a padded key space of 2^32 or more.                                             */
-enum { AXG_KEY_LINEAR = 0, AXG_KEY_BRICK = 1 };
+enum { AXG_KEY_LINEAR = 0, AXG_KEY_BRICK = 1, AXG_KEY_MORTON = 2 };
 int axg_set_key_order(axg_ctx* ctx, int order);
 
 /* Sensing rule of P3 (section 5.3: "each individual particle that the axon's
@@ -221,10 +242,43 @@ int axg_set_key_order(axg_ctx* ctx, int order);
  *                            near particles weigh more.
  * rint = round to nearest even.  Under both particle rules AXG_CONE_MOMENT is in units of 1/256 cell and
  * AXG_CONE_GRADIENT = G / (256 S2(R)); the sums stay integers (bit-exact, additive over shards, same sense buffer and
- * all-reduce), and P4 / P5 are unchanged.  Per cone the sums are int32 on the device: fewer than 2.7 M particles in
- * range.  Needs the binned state of P2 like the cell rule.  May be called between any two steps; bad mode: AXG_EINVAL. */
+ * all-reduce), and P4 / P5 are unchanged.  Per cone the sums are int32 on the device and are not checked for overflow: a
+ * moment component is bounded by n R (cell rule) or 256 n R (particle rules) for n particles in range, i.e. n must stay
+ * below 2^31 / R resp. 2^31 / (256 R) = 2.7 M at R = 3, 1.05 M at R = 8 (C1..C5: at most a few thousand).  Needs the binned state of P2 like the cell rule.  May be called between any two steps; bad mode: AXG_EINVAL. */
 enum { AXG_SENSE_CELL = 0, AXG_SENSE_PARTICLE = 1, AXG_SENSE_PARTICLE_WEIGHTED = 2 };
 int axg_set_sensing(axg_ctx* ctx, int mode);
+
+/* Connection formation (reading A-28).  PAPER.md:223-233 (section 3.3): "A collision
+ * takes place if the distance between the centres of the two spheres is less than the sum of the radii ... the algorithm
+ * will compare d^2 and the square of the sum of the radii"; the axon grows "until the end pivot of the
+ * capsule is in 0.05 units of another neuron"; the neurons "stored in a grid data structure entirely
+ * computed on the GPU" as the broadphase.
+ *  r_cone, r_soma   radii (cells) of the sphere around a growth-cone tip and around a soma (= the point where
+ *                   axg_place_neurons put the neuron); both >= 0, sum <= 64; sum 0 switches the rule off (default).
+ * Once on, every whole step ends with AXG_PHASE_CONNECT: each cone still ACTIVE after P5 is tested against the somata of
+ * all OTHER neurons, d2 = (dx dx + dy dy) + dz dz in fp32 (each operation rounded once), a hit iff d2 < fl(fl(r_cone +
+ * r_soma)^2); it connects to the nearest soma it hits (equal distances: the lowest index): AXG_CONE_TARGET[c] = that
+ * neuron, state AXG_CONE_CONNECTED, and it stops growing.  The somata are binned into a uniform grid of cubic cells whose
+ * edge is a power of two >= r_cone + r_soma, so a tip meets the somata of 27 cells only.  Sharded runs: replicated on
+ * every rank (same cones, same result).                                                                           */
+int axg_set_connect(axg_ctx* ctx, float r_cone, float r_soma);
+
+/* Harness hook: replace AXG_CONE_TARGET (n = the placed count; entries 0xffffffff or a neuron index other than the
+ * cone's own: AXG_EINVAL otherwise) so that the graph calls can be checked on given graphs.                         */
+int axg_load_targets(axg_ctx* ctx, const uint32_t* target, uint32_t n);
+
+/* The network as the paper's compact adjacency list (Fig. 4; reading A-29): vertex = neuron,
+ * every connected cone c is the edge c -> AXG_CONE_TARGET[c].  AXG_GRAPH_VA[i] is the head of vertex i's list in
+ * AXG_GRAPH_EA, the lists follow one another, AXG_GRAPH_VA[C] = E.  directed == 0: neighbours in either direction (the 0/1
+ * adjacency MATRIX the paper exports, Figs. 10-11, is symmetric); directed != 0: out-neighbours only.  Lists ascending,
+ * no duplicates.  AXG_ESTATE without neurons.  Synchronises.                                                       */
+int axg_build_graph(axg_ctx* ctx, int directed);
+
+/* Level-synchronous breadth-first search over the list of the last axg_build_graph (Fig. 5
+ * CUDA_BFS_KERNEL: one thread per vertex, frontier F_a, visited X_a, cost C_a, "repeated until frontier is empty";
+ * DESIGN.md reading A-30: with the second, updating frontier array of the algorithm the paper cites).  AXG_BFS_LEVEL[v] =
+ * number of edges from root, -1 if v is not reached.  AXG_ESTATE without a graph, AXG_EINVAL for a bad root.        */
+int axg_bfs(axg_ctx* ctx, uint32_t root);
 
 /* Device pointer (int32[C][AXG_MAX_SPECIES][4] = n,Mx,My,Mz) of the per-cone sensing sums, for the NCCL
  * all-reduce between P3 and P4 when sharded.  *bytes = its size.  Owned by ctx.                           */
@@ -242,6 +296,16 @@ int axg_sense_buffer(axg_ctx* ctx, void** device_ptr, size_t* bytes);
 int axg_check_capacity(axg_ctx* ctx, uint32_t n);
 int axg_enqueue_phase(axg_ctx* ctx, uint32_t phase_mask);
 int axg_sync(axg_ctx* ctx);
+
+/* The same, on a stream of the caller's choice (a cudaStream_t; the ctx stream is not touched), for the OVERLAPPED sharded
+ * step: P3, the all-reduce and P4 / P5 of step t on a side stream beside P1 of step t+1 on the main stream -- they share no
+ * data (P1 takes its step index from a counter of its own) -- joined by the caller's events before P2 of step t+1, exactly
+ * as axg_step orders one GPU's work.  overlapped != 0: the commit of these phases may run beside the NEXT step's P1 and must
+ * not re-align P1's step index (pass it for ADVANCE | COMMIT in that loop).  Capturable into a CUDA graph together with the
+ * NCCL all-reduce; axg_params_fingerprint changes whenever a captured launch would be stale (an allocation, a mode or a
+ * parameter changed).  paper_1405_3331_b200/sharded.py is the loop.                                                */
+int axg_enqueue_phase_on(axg_ctx* ctx, uint32_t phase_mask, void* stream, int overlapped);
+int axg_params_fingerprint(axg_ctx* ctx, uint64_t* fingerprint);
 
 /* Use `stream` (a cudaStream_t) for all later work of this ctx.                                          */
 int axg_set_stream(axg_ctx* ctx, void* stream);

@@ -17,15 +17,18 @@ FIELDS = dict(
     COUNTERS=0, PART_X=1, PART_Y=2, PART_Z=3, PART_SPECIES=4, PART_ID=5, KEYS_SORTED=6, PERM=7, CELL_START=8,
     CELL_END=9, CONE_POS=10, CONE_HEADING=11, CONE_STATE=12, CONE_COUNTS=13, CONE_MOMENT=14, CONE_GRADIENT=15,
     POLY_LEN=16, POLYLINE=17, PRE_X=18, PRE_Y=19, PRE_Z=20, PRE_SPECIES=21, PRE_ID=22, PRE_KEY=23,
+    CONE_TARGET=24, GRAPH_VA=25, GRAPH_EA=26, BFS_LEVEL=27,
 )
 _DTYPES = {
     0: np.uint64, 1: np.float32, 2: np.float32, 3: np.float32, 4: np.uint8, 5: np.uint32, 6: np.uint32, 7: np.uint32,
     8: np.uint32, 9: np.uint32, 10: np.float32, 11: np.float32, 12: np.uint8, 13: np.int64, 14: np.int64,
     15: np.float32, 16: np.uint32, 17: np.float32, 18: np.float32, 19: np.float32, 20: np.float32, 21: np.uint8,
-    22: np.uint32, 23: np.uint32,
+    22: np.uint32, 23: np.uint32, 24: np.uint32, 25: np.uint32, 26: np.uint32, 27: np.int32,
 }
 PHASE_DIFFUSE, PHASE_BIN, PHASE_SENSE, PHASE_ADVANCE, PHASE_COMMIT, PHASE_ALL = 1, 2, 4, 8, 16, 31
-COUNTER_NAMES = ("step", "n_live", "next_id", "emitted", "absorbed", "active", "arrived", "exited")
+PHASE_CONNECT = 32
+NO_TARGET = 0xFFFFFFFF
+COUNTER_NAMES = ("step", "n_live", "next_id", "emitted", "absorbed", "active", "arrived", "exited", "connected")
 
 
 class OracleError(RuntimeError):
@@ -58,6 +61,10 @@ def lib():
         L.axo_load_cones.argtypes = [vp, vp, vp, vp, vp, u32]
         L.axo_read_state.argtypes = [vp, u32, vp, C.c_size_t, C.POINTER(C.c_size_t)]
         L.axo_load_sense.argtypes = [vp, vp, vp, u32]
+        L.axo_set_connect.argtypes = [vp, f32, f32]
+        L.axo_load_targets.argtypes = [vp, vp, u32]
+        L.axo_build_graph.argtypes = [vp, C.c_int]
+        L.axo_bfs.argtypes = [vp, u32]
         L.axo_philox4x32_10.argtypes = [vp, vp, vp]
         L.axo_philox4x32_10.restype = None
         L.axo_normals.argtypes = [u64, u32, u32, u32, u32, vp, vp, vp]
@@ -120,6 +127,20 @@ class Oracle:
 
     def set_sensing(self, mode):
         self._chk(self._L.axo_set_sensing(self._h, int(mode)))
+
+    def set_connect(self, r_cone, r_soma):
+        self._chk(self._L.axo_set_connect(self._h, r_cone, r_soma))
+
+    def load_targets(self, target):
+        target = np.ascontiguousarray(target, dtype=np.uint32)
+        self._chk(self._L.axo_load_targets(self._h, _ptr(target), target.shape[0]))
+
+    def build_graph(self, directed=False):
+        self._chk(self._L.axo_build_graph(self._h, 1 if directed else 0))
+
+    def bfs(self, root):
+        self._chk(self._L.axo_bfs(self._h, int(root)))
+        return self.read_state("BFS_LEVEL")
 
     def set_shard(self, rank, world):
         self._chk(self._L.axo_set_shard(self._h, rank, world))

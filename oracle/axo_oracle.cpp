@@ -34,12 +34,14 @@ namespace {
 // ---- error codes / enums: restated here on purpose (no shared header with the CUDA path) -------------------
 enum { OK = 0, EINVAL_ = -1, ECAPACITY = -2, ESTATE = -3, ESMALL = -5 };
 enum { MAX_SPECIES = 4 };
-enum { CONE_ACTIVE = 0, CONE_ARRIVED = 1, CONE_EXITED = 2 };
-enum { PH_DIFFUSE = 1, PH_BIN = 2, PH_SENSE = 4, PH_ADVANCE = 8, PH_COMMIT = 16 };
+enum { CONE_ACTIVE = 0, CONE_ARRIVED = 1, CONE_EXITED = 2, CONE_CONNECTED = 3 };
+enum { PH_DIFFUSE = 1, PH_BIN = 2, PH_SENSE = 4, PH_ADVANCE = 8, PH_COMMIT = 16, PH_CONNECT = 32 };
+const uint32_t NO_TARGET = 0xffffffffu;
 enum Field {
     F_COUNTERS = 0, F_PART_X, F_PART_Y, F_PART_Z, F_PART_SPECIES, F_PART_ID, F_KEYS_SORTED, F_PERM, F_CELL_START,
     F_CELL_END, F_CONE_POS, F_CONE_HEADING, F_CONE_STATE, F_CONE_COUNTS, F_CONE_MOMENT, F_CONE_GRADIENT,
-    F_POLY_LEN, F_POLYLINE, F_PRE_X, F_PRE_Y, F_PRE_Z, F_PRE_SPECIES, F_PRE_ID, F_PRE_KEY, F_COUNT
+    F_POLY_LEN, F_POLYLINE, F_PRE_X, F_PRE_Y, F_PRE_Z, F_PRE_SPECIES, F_PRE_ID, F_PRE_KEY, F_CONE_TARGET, F_GRAPH_VA,
+    F_GRAPH_EA, F_BFS_LEVEL, F_COUNT
 };
 
 // ---- Philox4x32-10 (reading A-2; rationale for a stateless per-thread generator: §5.1) ------------
@@ -145,18 +147,46 @@ struct axo_ctx {
     std::vector<uint32_t> poly_len;
     std::vector<float> poly;  // C*(max_segments+1)*3 neuron-major
 
+    // connection formation (section 3.3, section 3.4; DESIGN.md readings
+    // A-28..A-30): target[c] = the neuron whose soma cone c has connected to (NO_TARGET: none), the adjacency list in
+    // the paper's compact form (Va = heads, Ea = edges) and the BFS levels of Fig. 5
+    bool connect_on = false;
+    float r_cone = 0.0f, r_soma = 0.0f;
+    std::vector<uint32_t> target;
+    std::vector<uint32_t> Va, Ea;
+    std::vector<int32_t> bfs_level;
+
     std::string err;
     // cell order ("a Z-order curve ... potential optimization"; reading A-27):
     // 0 = linear, x fastest (north_star); 1 = bricks of 8 x 4 x 4 cells, bricks in linear order (x fastest), cells inside
     // a brick in linear order (x fastest): key = brick * 128 + (z & 3) * 32 + (y & 3) * 8 + (x & 7).  The key space covers
     // the grid padded to whole bricks.
+    // 2 = Z-order (Morton) curve, the order P:263 names (reading A-31): the bits of ix, iy, iz interleaved from
+    // the least significant up, x first; a coordinate that has run out of bits (its axis needs fewer than the others)
+    // drops out of the rotation.  The key space is the grid padded to powers of two.
     int key_order = 0;
+    static int axis_bits(uint32_t n) {
+        int b = 0;
+        while ((1u << b) < n) ++b;
+        return b;
+    }
     size_t cells() const {
         if (key_order == 0) return (size_t)nx * ny * nz;
+        if (key_order == 2) return (size_t)1 << (axis_bits(nx) + axis_bits(ny) + axis_bits(nz));
         return (size_t)((nx + 7) / 8) * ((ny + 3) / 4) * ((nz + 3) / 4) * 128;
     }
     uint32_t key_of_cell(uint32_t ix, uint32_t iy, uint32_t iz) const {
         if (key_order == 0) return (iz * ny + iy) * nx + ix;
+        if (key_order == 2) {
+            const int nb[3] = {axis_bits(nx), axis_bits(ny), axis_bits(nz)};
+            const uint32_t v[3] = {ix, iy, iz};
+            uint32_t key = 0;
+            int out = 0;
+            for (int bit = 0; bit < 32; ++bit)          // bit `bit` of x, then of y, then of z, for the axes that have it
+                for (int a = 0; a < 3; ++a)
+                    if (bit < nb[a]) key |= ((v[a] >> bit) & 1u) << out++;
+            return key;
+        }
         const uint32_t nbx = (nx + 7) / 8, nby = (ny + 3) / 4;
         const uint32_t brick = ((iz / 4) * nby + (iy / 4)) * nbx + (ix / 8);
         return brick * 128 + (iz % 4) * 32 + (iy % 4) * 8 + (ix % 8);
@@ -449,6 +479,87 @@ void phase_advance(axo_ctx* c) {
     }
 }
 
+// Connection formation (reading A-28).  P:223-233: "A collision takes place if the distance between the centres
+// of the two spheres is less than the sum of the radii ... the algorithm will compare d^2 and the square of the sum of
+// the radii"; the axon grows "until the end pivot of the capsule is in 0.05 units of another neuron".  Plain
+// definition, all pairs: every cone that is still ACTIVE after O9 is tested against the soma (= first polyline point)
+// of every OTHER neuron; of the somata it touches it connects to the nearest (ties: the lowest index) and stops growing.
+// fp32 decides an integer here, so the precision and order are part of the reading: d = tip - soma per axis,
+// d2 = (dx dx + dy dy) + dz dz, each operation rounded once, compared (strictly) with fl(fl(r_cone + r_soma)^2).
+void phase_connect(axo_ctx* c) {
+    if (!c->connect_on) return;
+    const size_t stride = (size_t)(c->max_segments + 1) * 3;
+    const float reach = c->r_cone + c->r_soma;
+    const float thr = reach * reach;
+    if (c->target.size() != c->n_cones()) c->target.assign(c->n_cones(), NO_TARGET);
+    for (size_t cone = 0; cone < c->n_cones(); ++cone) {
+        if (c->cone_state[cone] != CONE_ACTIVE) continue;
+        const float* p = &c->cone_pos[cone * 3];
+        float best = 0.0f;
+        uint32_t who = NO_TARGET;
+        for (size_t n = 0; n < c->n_cones(); ++n) {
+            if (n == cone) continue;  // not its own neuron
+            const float* s = &c->poly[n * stride];
+            const float dx = p[0] - s[0], dy = p[1] - s[1], dz = p[2] - s[2];
+            const float d2 = (dx * dx + dy * dy) + dz * dz;
+            if (d2 < thr && (who == NO_TARGET || d2 < best)) {
+                best = d2;
+                who = (uint32_t)n;
+            }
+        }
+        if (who != NO_TARGET) {
+            c->target[cone] = who;
+            c->cone_state[cone] = CONE_CONNECTED;
+        }
+    }
+}
+
+// The adjacency list of the network in the paper's compact form (Fig. 4; reading A-29): vertex = neuron,
+// Va[i] = head of vertex i's list in Ea, "edges of vertex i+1 following the edges of vertex i", Va[N] = |Ea|.  Every
+// connected cone c gives the edge c -> target[c]; undirected (the adjacency MATRIX of Figs. 10/11 is what the paper
+// exports): i and j are neighbours if either has connected to the other.  Lists ascending, no duplicates.
+void build_graph(axo_ctx* c, bool directed) {
+    const size_t N = c->n_cones();
+    if (c->target.size() != N) c->target.assign(N, NO_TARGET);
+    std::vector<std::vector<uint32_t>> adj(N);
+    for (size_t i = 0; i < N; ++i) {
+        const uint32_t t = c->target[i];
+        if (t == NO_TARGET) continue;
+        adj[i].push_back(t);
+        if (!directed) adj[t].push_back((uint32_t)i);
+    }
+    c->Va.assign(N + 1, 0u);
+    c->Ea.clear();
+    for (size_t i = 0; i < N; ++i) {
+        std::sort(adj[i].begin(), adj[i].end());
+        adj[i].erase(std::unique(adj[i].begin(), adj[i].end()), adj[i].end());
+        c->Va[i] = (uint32_t)c->Ea.size();
+        c->Ea.insert(c->Ea.end(), adj[i].begin(), adj[i].end());
+    }
+    c->Va[N] = (uint32_t)c->Ea.size();
+}
+
+// Breadth-first levels from `root` over (Va, Ea): what Fig. 5's CUDA_BFS_KERNEL computes level by level (C_a = cost =
+// number of edges from the root), written here as the textbook queue BFS the paper contrasts it with.
+// Unreached vertices: -1.
+void bfs(axo_ctx* c, uint32_t root) {
+    const size_t N = c->n_cones();
+    c->bfs_level.assign(N, -1);
+    std::vector<uint32_t> queue;
+    queue.push_back(root);
+    c->bfs_level[root] = 0;
+    for (size_t head = 0; head < queue.size(); ++head) {
+        const uint32_t v = queue[head];
+        for (uint32_t e = c->Va[v]; e < c->Va[v + 1]; ++e) {
+            const uint32_t w = c->Ea[e];
+            if (c->bfs_level[w] < 0) {
+                c->bfs_level[w] = c->bfs_level[v] + 1;
+                queue.push_back(w);
+            }
+        }
+    }
+}
+
 int run_phases(axo_ctx* c, uint32_t mask) {
     if (mask & PH_DIFFUSE) phase_diffuse(c);
     if (mask & PH_BIN) {
@@ -457,6 +568,7 @@ int run_phases(axo_ctx* c, uint32_t mask) {
     }
     if (mask & PH_SENSE) phase_sense(c);
     if (mask & PH_ADVANCE) phase_advance(c);
+    if (mask & PH_CONNECT) phase_connect(c);
     if (mask & PH_COMMIT) c->step += 1;  // O10
     c->stepped = true;
     return OK;
@@ -555,6 +667,8 @@ AXO_API int axo_place_neurons(axo_ctx* c, const float* xyz, const float* heading
     c->poly.assign((size_t)n * stride, 0.0f);
     for (uint32_t i = 0; i < n; ++i)
         for (int a = 0; a < 3; ++a) c->poly[i * stride + a] = xyz[i * 3 + a];
+    c->target.assign(n, NO_TARGET);
+    c->Va.clear(); c->Ea.clear(); c->bfs_level.clear();
     return OK;
 }
 
@@ -579,7 +693,7 @@ AXO_API int axo_set_shard(axo_ctx* c, uint32_t rank, uint32_t world) {
 
 // 0 = linear cell order (default), 1 = bricks of 8 x 4 x 4 cells (reading A-27); only before any particle exists
 AXO_API int axo_set_key_order(axo_ctx* c, int order) {
-    if (!c || (order != 0 && order != 1)) return fail(c, EINVAL_, "bad key order");
+    if (!c || (order < 0 || order > 2)) return fail(c, EINVAL_, "bad key order");
     if (c->stepped || c->A.size() || c->B.size()) return fail(c, ESTATE, "key order must be set before particles exist");
     c->key_order = order;
     c->cell_start.clear(); c->cell_end.clear();
@@ -616,12 +730,13 @@ AXO_API int axo_step(axo_ctx* c, uint32_t n) {
     if (!c) return EINVAL_;
     const int rc = capacity_check(c, n, true, true);
     if (rc) return rc;
-    for (uint32_t i = 0; i < n; ++i) run_phases(c, PH_DIFFUSE | PH_BIN | PH_SENSE | PH_ADVANCE | PH_COMMIT);
+    for (uint32_t i = 0; i < n; ++i)
+        run_phases(c, PH_DIFFUSE | PH_BIN | PH_SENSE | PH_ADVANCE | PH_COMMIT | (c->connect_on ? PH_CONNECT : 0));
     return OK;
 }
 
 AXO_API int axo_step_phase(axo_ctx* c, uint32_t mask) {
-    if (!c || (mask & ~31u)) return fail(c, EINVAL_, "bad phase mask");
+    if (!c || (mask & ~63u)) return fail(c, EINVAL_, "bad phase mask");
     const int rc = capacity_check(c, 1, mask & PH_DIFFUSE, mask & PH_ADVANCE);
     if (rc) return rc;
     return run_phases(c, mask);
@@ -657,9 +772,9 @@ AXO_API int axo_read_state(axo_ctx* c, uint32_t field, void* dst, size_t dst_byt
     if (!c) return EINVAL_;
     switch (field) {
         case F_COUNTERS: {
-            uint64_t v[8] = {c->step, c->n_live, c->next_id, c->emitted, c->absorbed, 0, 0, 0};
-            for (size_t i = 0; i < c->n_cones(); ++i) v[5 + c->cone_state[i]] += 1;
-            return copy_out(c, v, 8, dst, dst_bytes, n_elems);
+            uint64_t v[9] = {c->step, c->n_live, c->next_id, c->emitted, c->absorbed, 0, 0, 0, 0};
+            for (size_t i = 0; i < c->n_cones(); ++i) v[5 + c->cone_state[i]] += 1;  // active, arrived, exited, connected
+            return copy_out(c, v, 9, dst, dst_bytes, n_elems);
         }
         case F_PART_X: return copy_out(c, c->A.x.data(), c->A.size(), dst, dst_bytes, n_elems);
         case F_PART_Y: return copy_out(c, c->A.y.data(), c->A.size(), dst, dst_bytes, n_elems);
@@ -691,8 +806,47 @@ AXO_API int axo_read_state(axo_ctx* c, uint32_t field, void* dst, size_t dst_byt
         case F_PRE_SPECIES: return copy_out(c, c->B.species.data(), c->B.size(), dst, dst_bytes, n_elems);
         case F_PRE_ID: return copy_out(c, c->B.id.data(), c->B.size(), dst, dst_bytes, n_elems);
         case F_PRE_KEY: return copy_out(c, c->key.data(), c->key.size(), dst, dst_bytes, n_elems);
+        case F_CONE_TARGET:
+            if (c->target.size() != c->n_cones()) c->target.assign(c->n_cones(), NO_TARGET);
+            return copy_out(c, c->target.data(), c->target.size(), dst, dst_bytes, n_elems);
+        case F_GRAPH_VA: return copy_out(c, c->Va.data(), c->Va.size(), dst, dst_bytes, n_elems);
+        case F_GRAPH_EA: return copy_out(c, c->Ea.data(), c->Ea.size(), dst, dst_bytes, n_elems);
+        case F_BFS_LEVEL: return copy_out(c, c->bfs_level.data(), c->bfs_level.size(), dst, dst_bytes, n_elems);
         default: return fail(c, EINVAL_, "unknown field");
     }
+}
+
+AXO_API int axo_set_connect(axo_ctx* c, float r_cone, float r_soma) {
+    if (!c || !(r_cone >= 0.0f) || !(r_soma >= 0.0f) || !std::isfinite(r_cone) || !std::isfinite(r_soma))
+        return fail(c, EINVAL_, "bad radii");
+    c->connect_on = (r_cone + r_soma) > 0.0f;
+    c->r_cone = r_cone;
+    c->r_soma = r_soma;
+    return OK;
+}
+
+// harness hook: replace the connection targets (graph / BFS checked on given graphs)
+AXO_API int axo_load_targets(axo_ctx* c, const uint32_t* target, uint32_t n) {
+    if (!c || (!target && n)) return fail(c, EINVAL_, "null argument");
+    if (n != c->n_cones()) return fail(c, EINVAL_, "cone count differs from the placed count");
+    for (uint32_t i = 0; i < n; ++i)
+        if (target[i] != NO_TARGET && (target[i] >= n || target[i] == i)) return fail(c, EINVAL_, "bad target");
+    c->target.assign(target, target + n);
+    return OK;
+}
+
+AXO_API int axo_build_graph(axo_ctx* c, int directed) {
+    if (!c) return EINVAL_;
+    build_graph(c, directed != 0);
+    return OK;
+}
+
+AXO_API int axo_bfs(axo_ctx* c, uint32_t root) {
+    if (!c) return EINVAL_;
+    if (c->Va.size() != c->n_cones() + 1) return fail(c, ESTATE, "no graph: call axo_build_graph first");
+    if (root >= c->n_cones()) return fail(c, EINVAL_, "root out of range");
+    bfs(c, root);
+    return OK;
 }
 
 // Harness-only load hook for the sharded loop (world_size-2 gloo tests): replace the per-cone sums of the last P3

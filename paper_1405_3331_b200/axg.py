@@ -17,20 +17,23 @@ FIELDS = dict(
     COUNTERS=0, PART_X=1, PART_Y=2, PART_Z=3, PART_SPECIES=4, PART_ID=5, KEYS_SORTED=6, PERM=7, CELL_START=8,
     CELL_END=9, CONE_POS=10, CONE_HEADING=11, CONE_STATE=12, CONE_COUNTS=13, CONE_MOMENT=14, CONE_GRADIENT=15,
     POLY_LEN=16, POLYLINE=17, PRE_X=18, PRE_Y=19, PRE_Z=20, PRE_SPECIES=21, PRE_ID=22, PRE_KEY=23,
+    CONE_TARGET=24, GRAPH_VA=25, GRAPH_EA=26, BFS_LEVEL=27,
 )
 _DTYPES = {
     0: np.uint64, 1: np.float32, 2: np.float32, 3: np.float32, 4: np.uint8, 5: np.uint32, 6: np.uint32, 7: np.uint32,
     8: np.uint32, 9: np.uint32, 10: np.float32, 11: np.float32, 12: np.uint8, 13: np.int64, 14: np.int64,
     15: np.float32, 16: np.uint32, 17: np.float32, 18: np.float32, 19: np.float32, 20: np.float32, 21: np.uint8,
-    22: np.uint32, 23: np.uint32,
+    22: np.uint32, 23: np.uint32, 24: np.uint32, 25: np.uint32, 26: np.uint32, 27: np.int32,
 }
 PHASE_DIFFUSE, PHASE_BIN, PHASE_SENSE, PHASE_ADVANCE, PHASE_COMMIT, PHASE_ALL = 1, 2, 4, 8, 16, 31
-COUNTER_NAMES = ("step", "n_live", "next_id", "emitted", "absorbed", "active", "arrived", "exited")
+PHASE_CONNECT = 32
+NO_TARGET = 0xFFFFFFFF
+COUNTER_NAMES = ("step", "n_live", "next_id", "emitted", "absorbed", "active", "arrived", "exited", "connected")
 KERNEL_NAMES = ("clear", "diffuse", "emit", "sort", "reorder", "sense", "advance", "commit", "scan", "place", "settle")
 BIN_AUTO, BIN_RADIX, BIN_COUNT = 0, 1, 2
 STEER_VECTOR, STEER_SNR = 0, 1
 SENSE_CELL, SENSE_PARTICLE, SENSE_PARTICLE_WEIGHTED = 0, 1, 2
-KEY_LINEAR, KEY_BRICK = 0, 1
+KEY_LINEAR, KEY_BRICK, KEY_MORTON = 0, 1, 2
 AUTO_COUNT_MAX_CELLS = 1 << 31   # include/axg.h AXG_AUTO_COUNT_MAX_CELLS
 EXPORTS = (
     "axg_create", "axg_place_neurons", "axg_add_source", "axg_step", "axg_read_state", "axg_destroy",
@@ -40,6 +43,9 @@ EXPORTS = (
     "axg_set_steering",
     "axg_set_sensing",
     "axg_set_key_order",
+    "axg_get_binning",
+    "axg_set_connect", "axg_load_targets", "axg_build_graph", "axg_bfs",
+    "axg_enqueue_phase_on", "axg_params_fingerprint",
 )
 
 _ALLOC_T = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p)
@@ -89,7 +95,14 @@ def lib(build=True):
     L.axg_check_capacity.argtypes = [vp, u32]
     L.axg_enqueue_phase.argtypes = [vp, u32]
     L.axg_sync.argtypes = [vp]
+    L.axg_enqueue_phase_on.argtypes = [vp, u32, vp, C.c_int]
+    L.axg_params_fingerprint.argtypes = [vp, C.POINTER(u64)]
     L.axg_set_binning.argtypes = [vp, C.c_int]
+    L.axg_get_binning.argtypes = [vp, C.POINTER(C.c_int)]
+    L.axg_set_connect.argtypes = [vp, f32, f32]
+    L.axg_load_targets.argtypes = [vp, vp, u32]
+    L.axg_build_graph.argtypes = [vp, C.c_int]
+    L.axg_bfs.argtypes = [vp, u32]
     L.axg_set_steering.argtypes = [vp, C.c_int, C.c_float, C.c_float]
     L.axg_set_sensing.argtypes = [vp, C.c_int]
     L.axg_set_key_order.argtypes = [vp, C.c_int]
@@ -192,6 +205,11 @@ class Axg:
     def set_binning(self, mode):
         self._chk(self._L.axg_set_binning(self._h, int(mode)))
 
+    def get_binning(self):
+        mode = C.c_int(0)
+        self._chk(self._L.axg_get_binning(self._h, C.byref(mode)))
+        return mode.value
+
     def set_key_order(self, order):
         self._chk(self._L.axg_set_key_order(self._h, int(order)))
 
@@ -200,6 +218,20 @@ class Axg:
 
     def set_steering(self, mode, gain=1.0, turn=3.141592653589793 / 30):
         self._chk(self._L.axg_set_steering(self._h, int(mode), gain, turn))
+
+    def set_connect(self, r_cone, r_soma):
+        self._chk(self._L.axg_set_connect(self._h, r_cone, r_soma))
+
+    def load_targets(self, target):
+        target = np.ascontiguousarray(target, dtype=np.uint32)
+        self._chk(self._L.axg_load_targets(self._h, _ptr(target), target.shape[0]))
+
+    def build_graph(self, directed=False):
+        self._chk(self._L.axg_build_graph(self._h, 1 if directed else 0))
+
+    def bfs(self, root):
+        self._chk(self._L.axg_bfs(self._h, int(root)))
+        return self.read_state("BFS_LEVEL")
 
     def set_shard(self, rank, world):
         self._chk(self._L.axg_set_shard(self._h, rank, world))
@@ -218,6 +250,14 @@ class Axg:
 
     def sync(self):
         self._chk(self._L.axg_sync(self._h))
+
+    def enqueue_phase_on(self, mask, cuda_stream, overlapped=False):
+        self._chk(self._L.axg_enqueue_phase_on(self._h, mask, int(cuda_stream), 1 if overlapped else 0))
+
+    def params_fingerprint(self):
+        fp = C.c_uint64(0)
+        self._chk(self._L.axg_params_fingerprint(self._h, C.byref(fp)))
+        return fp.value
 
     def load_particles(self, x, y, z, species, ids, next_id, step):
         x = np.ascontiguousarray(x, dtype=np.float32)

@@ -91,11 +91,28 @@ struct axg_ctx {
     float ktimes[AXG_KERNEL_COUNT] = {0};
     std::vector<cudaEvent_t> prof_events;
 
+    // connection formation / graph (axg_set_connect, axg_build_graph, axg_bfs)
+    float r_cone = 0.f, r_soma = 0.f;
+    bool soma_grid_built = false;
+    std::vector<void*> connect_bufs;   // soma grid
+    void* d_target = nullptr;
+    std::vector<void*> graph_bufs;
+    AxgGraph G;
+    bool graph_built = false;
+    uint32_t graph_edges = 0;
+    bool bfs_done = false;
+
     int key_order = AXG_KEY_LINEAR;  // axg_set_key_order: AXG_KEY_BRICK pads the key space to whole 8 x 4 x 4 bricks
     size_t nbx() const { return (grid.nx + 7) / 8; }
     size_t nby() const { return (grid.ny + 3) / 4; }
+    static int axis_bits(uint32_t n) {
+        int b = 0;
+        while ((1u << b) < n) ++b;
+        return b;
+    }
     size_t cells() const {  // size of the key space
         if (key_order == AXG_KEY_LINEAR) return (size_t)grid.nx * grid.ny * grid.nz;
+        if (key_order == AXG_KEY_MORTON) return (size_t)1 << (axis_bits(grid.nx) + axis_bits(grid.ny) + axis_bits(grid.nz));
         return nbx() * nby() * ((grid.nz + 3) / 4) * 128;
     }
     // cell arrays are padded to whole scan tiles so that 128-bit accesses of the last tile stay inside
@@ -105,6 +122,8 @@ struct axg_ctx {
 };
 
 namespace {
+
+int ensure_soma_grid(axg_ctx* c);  // connection formation, defined with the graph calls below
 
 int fail(axg_ctx* c, int code, const std::string& msg) {
     if (c) c->err = msg; else g_create_err = msg;
@@ -188,6 +207,25 @@ int alloc_fixed(axg_ctx* c) {
     P.cell_lo = (uint32_t*)c->d_cell_lo;
     P.nx = c->grid.nx; P.ny = c->grid.ny; P.nz = c->grid.nz; P.cells = (uint32_t)c->cells();
     P.key_order = c->key_order; P.nbx = (uint32_t)c->nbx(); P.nby = (uint32_t)c->nby();
+    {   // the phases of the Z-order bit rotation (reading A-31)
+        const int nb[3] = {axg_ctx::axis_bits(c->grid.nx), axg_ctx::axis_bits(c->grid.ny), axg_ctx::axis_bits(c->grid.nz)};
+        const int m3 = std::min(nb[0], std::min(nb[1], nb[2]));
+        int rem[3], left[3], n_left = 0;
+        for (int a = 0; a < 3; ++a) {
+            rem[a] = nb[a] - m3;
+            if (rem[a] > 0) left[n_left++] = a;
+        }
+        P.mo_m3 = (uint32_t)m3; P.mo_m2 = 0; P.mo_p = 0; P.mo_q = 1; P.mo_r = 0; P.mo_rshift = 0; P.mo_rbits = 0;
+        if (n_left == 2) {
+            const int pa = left[0], qa = left[1], m2 = std::min(rem[pa], rem[qa]);
+            P.mo_p = (uint32_t)pa; P.mo_q = (uint32_t)qa; P.mo_m2 = (uint32_t)m2;
+            P.mo_r = (uint32_t)(rem[pa] >= rem[qa] ? pa : qa);
+            P.mo_rshift = (uint32_t)(m3 + m2);
+            P.mo_rbits = (uint32_t)std::abs(rem[pa] - rem[qa]);
+        } else if (n_left == 1) {
+            P.mo_r = (uint32_t)left[0]; P.mo_rshift = (uint32_t)m3; P.mo_rbits = (uint32_t)rem[left[0]];
+        }
+    }
     P.fnx = (float)c->grid.nx; P.fny = (float)c->grid.ny; P.fnz = (float)c->grid.nz;
     P.sigma = (float)std::sqrt(2.0 * (double)c->D);  // O0
     P.seed_lo = (uint32_t)(c->seed & 0xffffffffull);
@@ -220,10 +258,10 @@ int alloc_particles(axg_ctx* c, uint64_t cap, AxgParams& P, std::vector<void*>& 
     const size_t diff_tiles = n / axg_diffuse_tile() + 2, sort_tiles = n / axg_sort_tile() + 2;
     const size_t sizes[] = {n * 4, n * 4, n * 4, n, n * 4,  // A (SoA)
                             n * 16, n,                      // Brec, Bsp
-                            n * 4, n * 4, n * 4, n * 4, n * 4,  // key_pre, skey[2], sidx[2]
+                            n * 8, n * 4, n * 4, n * 4, n * 4,  // key_pre (radix) = kw (count: key + arrival rank), skey[2], sidx[2]
                             diff_tiles * 8, sort_tiles * AXG_RADIX * 8,
                             (n / AXG_CHUNK + 4) * 4, (n / AXG_CHUNK + 4) * 4,   // chunk_cnt, chunk_base
-                            n * 4, AXG_MAX_SOURCES * 4};                        // arr_pre, src_arr
+                            (n / 33 + 64) * 4, AXG_MAX_SOURCES * 4};            // big_list, src_arr
     constexpr int NB = 18;
     void* ptr[NB];
     for (int i = 0; i < NB; ++i) {
@@ -245,7 +283,8 @@ int alloc_particles(axg_ctx* c, uint64_t cap, AxgParams& P, std::vector<void*>& 
     P.sort_state = (unsigned long long*)ptr[13];
     P.chunk_cnt = (uint32_t*)ptr[14];
     P.chunk_base = (uint32_t*)ptr[15];
-    P.arr_pre = (uint32_t*)ptr[16];
+    P.kw = (uint2*)ptr[7];
+    P.big_list = (uint32_t*)ptr[16];
     P.src_arr = (uint32_t*)ptr[17];
     P.capacity = (uint32_t)cap;
     // look-back words must not alias a live epoch: zero them (epoch 0 words with flag 0 = not ready)
@@ -286,7 +325,26 @@ int ensure_particles(axg_ctx* c) {
     return resolve_binning(c);
 }
 
+void free_graph(axg_ctx* c) {
+    for (void* p : c->graph_bufs) dev_free(p);
+    c->graph_bufs.clear();
+    c->graph_built = c->bfs_done = false;
+    c->graph_edges = 0;
+}
+
+void free_connect(axg_ctx* c) {
+    for (void* p : c->connect_bufs) dev_free(p);
+    c->connect_bufs.clear();
+    c->soma_grid_built = false;
+    c->P.ng_lo = nullptr;
+    c->P.ng_list = nullptr;
+}
+
 void free_cones(axg_ctx* c) {
+    free_graph(c);
+    free_connect(c);
+    dev_free(c->d_target);
+    c->d_target = nullptr;
     for (void* p : c->cone_bufs) dev_free(p);
     c->cone_bufs.clear();
     dev_free(c->d_poly);
@@ -315,6 +373,10 @@ int alloc_cones(axg_ctx* c, uint32_t n) {
     c->d_poly = dev_alloc(c, poly_bytes(c, c->max_segments));
     if (!c->d_poly) return fail(c, AXG_ECUDA, "device allocation failed (polylines)");
     CU(c, cudaMemsetAsync(c->d_poly, 0, poly_bytes(c, c->max_segments), c->stream));
+    c->d_target = dev_alloc(c, (size_t)n * 4);
+    if (!c->d_target) return fail(c, AXG_ECUDA, "device allocation failed (cone targets)");
+    CU(c, cudaMemsetAsync(c->d_target, 0xff, (size_t)n * 4, c->stream));  // 0xffffffff = no connection
+    P.cone_target = (uint32_t*)c->d_target;
     P.cone_pos = (float*)ptr[0]; P.cone_heading = (float*)ptr[1]; P.cone_state = (uint8_t*)ptr[2];
     P.sense = (int32_t*)ptr[3]; P.cone_gradient = (float*)ptr[4]; P.poly_len = (uint32_t*)ptr[5];
     P.poly = (float*)c->d_poly;
@@ -384,9 +446,12 @@ struct Prof {
 };
 
 // enqueue the selected phases of one step; returns the number of kernel launches
-int enqueue_phases(axg_ctx* c, uint32_t mask, Prof& prof, bool overlap = false) {
+// on / no_realign: the sharded loop's form (axg_enqueue_phase_on) -- the phases go to the stream `on`, and a commit that
+// runs beside the next step's P1 must not re-align P1's step index (P1 has already bumped it)
+int enqueue_phases(axg_ctx* c, uint32_t mask, Prof& prof, bool overlap = false, cudaStream_t on = nullptr,
+                   bool use_on = false, bool no_realign = false) {
     const AxgParams& P = c->P;
-    cudaStream_t s = c->stream;
+    cudaStream_t s = use_on ? on : c->stream;
     int launches = 0;
     const bool count_mode = P.bin_mode == AXG_BIN_COUNT_D;
     auto zero_cnt_if_dirty = [&]() {  // harness orders only (P1 twice, or P2 on given positions after a P1)
@@ -449,6 +514,10 @@ int enqueue_phases(axg_ctx* c, uint32_t mask, Prof& prof, bool overlap = false) 
         axg_launch_advance(P, committed ? 1 : 0, sc);
         launches += 1;
     }
+    if ((mask & AXG_PHASE_CONNECT) && P.n_cones && P.conn_thr > 0.0f) {  // reading A-28: after O9, before the next step
+        axg_launch_connect(P, sc);
+        launches += 1;
+    }
     if (overlap) {
         cudaEventRecord(c->ev_adv, c->side);
         c->adv_pending = true;
@@ -457,7 +526,7 @@ int enqueue_phases(axg_ctx* c, uint32_t mask, Prof& prof, bool overlap = false) 
         prof.mark(AXG_K_COMMIT);
         axg_launch_commit(P, 1, s);
         launches += 1;
-    } else if (committed && !(mask & AXG_PHASE_DIFFUSE)) {  // phase calls: keep P1's step index aligned
+    } else if (committed && !(mask & AXG_PHASE_DIFFUSE) && !no_realign) {  // phase calls: keep P1's step index aligned
         axg_launch_commit(P, 0, sc);
         launches += 1;
     }
@@ -477,8 +546,12 @@ int enqueue_unit(axg_ctx* c, cudaStream_t s, bool prev_cones) {
         cudaStreamWaitEvent(c->side, c->ev_bin, 0);
         axg_launch_sense(P, c->side);
         axg_launch_advance(P, 1, c->side);  // O10 rides in its last block
-        cudaEventRecord(c->ev_adv, c->side);
         launches += 2;
+        if (P.conn_thr > 0.0f) {
+            axg_launch_connect(P, c->side);
+            launches += 1;
+        }
+        cudaEventRecord(c->ev_adv, c->side);
     }
     axg_launch_diffuse(P, N_SM * 4, s);
     if (prev_cones) cudaStreamWaitEvent(s, c->ev_adv, 0);
@@ -537,7 +610,8 @@ long long enqueue_steps_graph(axg_ctx* c, uint32_t n) {
         c->graph_stream = s;
         c->graph_cones = cones;
     } else {
-        unit_launches = (c->P.bin_mode == AXG_BIN_COUNT_D ? 4 : c->P.n_pass + 2) + (cones ? 2 : 1);
+        unit_launches = (c->P.bin_mode == AXG_BIN_COUNT_D ? 4 : c->P.n_pass + 2) +
+                        (cones ? 2 + (c->P.conn_thr > 0.0f ? 1 : 0) : 1);
     }
     if (detour) {
         cudaEventRecord(c->ev_fork, c->stream);
@@ -556,6 +630,10 @@ long long enqueue_steps_graph(axg_ctx* c, uint32_t n) {
         axg_launch_sense(c->P, s);
         axg_launch_advance(c->P, 1, s);
         launches += 2;
+        if (c->P.conn_thr > 0.0f) {
+            axg_launch_connect(c->P, s);
+            launches += 1;
+        }
     }
     if (detour) {
         cudaEventRecord(c->ev_join, s);
@@ -581,7 +659,7 @@ void finish_prof(axg_ctx* c, Prof& prof) {
 int capacity_check(axg_ctx* c, uint32_t n, bool diffuse, bool advance, AxgDev* h) {
     const bool census = advance && c->n_cones;
     if (census) {  // longest active polyline, on the stream ahead of the one read below: one synchronisation, not two
-        CU(c, cudaMemsetAsync(&((AxgDev*)c->d_dev)->cone_census[0], 0, 4 * sizeof(uint32_t), c->stream));
+        CU(c, cudaMemsetAsync(&((AxgDev*)c->d_dev)->cone_census[0], 0, 5 * sizeof(uint32_t), c->stream));
         axg_launch_census(c->P, c->stream);
     }
     int rc = read_dev(c, h);
@@ -591,6 +669,21 @@ int capacity_check(axg_ctx* c, uint32_t n, bool diffuse, bool advance, AxgDev* h
     if (census && h->cone_census[0] && (uint64_t)h->cone_census[3] + n > (uint64_t)c->max_segments + 1)
         return fail(c, AXG_ECAPACITY, "polyline capacity would overflow");
     return AXG_OK;
+}
+
+// The device error word, read after a synchronisation: report it ONCE and clear it, so that a context whose capacity
+// has been raised (or whose particles have been replaced) works again.  Bits: 1 particle capacity, 2 polyline
+// capacity (both: the step that hit them dropped its emission / its append -- the state is no longer the one an
+// unbounded run would have), 4 a loaded particle outside the domain reached AXG_PHASE_BIN (k_rekey).
+int report_dev_err(axg_ctx* c, const AxgDev& h) {
+    if (!h.err) return AXG_OK;
+    cudaMemsetAsync(&((AxgDev*)c->d_dev)->err, 0, sizeof(uint32_t), c->stream);
+    cudaStreamSynchronize(c->stream);
+    char msg[160];
+    std::snprintf(msg, sizeof msg,
+                  "device error word 0x%x (1 = particle capacity, 2 = polyline capacity, 4 = particle outside the domain); "
+                  "the state is undefined: reload it", h.err);
+    return fail(c, (h.err & 3u) ? AXG_ECAPACITY : AXG_EINVAL, msg);
 }
 
 int after_sync(axg_ctx* c, const char* what) {
@@ -676,6 +769,14 @@ AXG_API int axg_set_binning(axg_ctx* c, int mode) {
     return c->particles_allocated ? resolve_binning(c) : AXG_OK;
 }
 
+AXG_API int axg_get_binning(axg_ctx* c, int* mode) {
+    if (!c || !mode) return fail(c, AXG_EINVAL, "null argument");
+    const int rc = ensure_particles(c);
+    if (rc) return rc;
+    *mode = c->P.bin_mode == AXG_BIN_COUNT_D ? AXG_BIN_COUNT : AXG_BIN_RADIX;
+    return AXG_OK;
+}
+
 AXG_API int axg_set_steering(axg_ctx* c, int mode, float gain, float turn) {
     if (!c || (mode != AXG_STEER_VECTOR && mode != AXG_STEER_SNR) || !(gain >= 0.0f) || !std::isfinite(gain) ||
         !(turn > 0.0f) || !(turn < 3.14159265f))
@@ -688,11 +789,15 @@ AXG_API int axg_set_steering(axg_ctx* c, int mode, float gain, float turn) {
 }
 
 AXG_API int axg_set_key_order(axg_ctx* c, int order) {
-    if (!c || (order != AXG_KEY_LINEAR && order != AXG_KEY_BRICK)) return fail(c, AXG_EINVAL, "bad key order");
+    if (!c || (order != AXG_KEY_LINEAR && order != AXG_KEY_BRICK && order != AXG_KEY_MORTON))
+        return fail(c, AXG_EINVAL, "bad key order");
     if (order == c->key_order) return AXG_OK;
     if (c->d_dev) return fail(c, AXG_ESTATE, "the key order must be set directly after axg_create");
     const size_t brick_cells = c->nbx() * c->nby() * ((c->grid.nz + 3) / 4) * 128;
     if (order == AXG_KEY_BRICK && brick_cells >= (1ull << 32)) return fail(c, AXG_EINVAL, "padded key space >= 2^32");
+    if (order == AXG_KEY_MORTON && axg_ctx::axis_bits(c->grid.nx) + axg_ctx::axis_bits(c->grid.ny) +
+                                       axg_ctx::axis_bits(c->grid.nz) > 31)
+        return fail(c, AXG_EINVAL, "padded key space >= 2^32");
     c->key_order = order;
     return AXG_OK;
 }
@@ -743,7 +848,8 @@ AXG_API int axg_place_neurons(axg_ctx* c, const float* xyz, const float* heading
     CU(c, cudaMemcpyAsync(c->P.cone_heading, hd.data(), (size_t)n * 12, cudaMemcpyHostToDevice, c->stream));
     CU(c, cudaMemcpyAsync(c->P.poly_len, ones.data(), (size_t)n * 4, cudaMemcpyHostToDevice, c->stream));
     axg_launch_poly_init(c->P, c->stream);
-    return after_sync(c, "axg_place_neurons");
+    rc = after_sync(c, "axg_place_neurons");
+    return rc ? rc : ensure_soma_grid(c);
 }
 
 AXG_API int axg_set_capacity(axg_ctx* c, uint64_t max_particles, uint32_t max_segments) {
@@ -794,6 +900,7 @@ AXG_API int axg_set_capacity(axg_ctx* c, uint64_t max_particles, uint32_t max_se
         c->kp_pending = false;
     }
     c->max_particles = max_particles;
+    CU(c, cudaMemsetAsync(&((AxgDev*)c->d_dev)->err, 0, sizeof(uint32_t), c->stream));
     return c->particles_allocated ? resolve_binning(c) : AXG_OK;  // AXG_BIN_AUTO depends on the capacity
 }
 
@@ -827,6 +934,7 @@ AXG_API int axg_load_particles(axg_ctx* c, const float* x, const float* y, const
     CU(c, cudaMemcpyAsync(&d->next_id, &next_id, 4, cudaMemcpyHostToDevice, c->stream));
     CU(c, cudaMemcpyAsync(&d->step, &step, 4, cudaMemcpyHostToDevice, c->stream));
     CU(c, cudaMemcpyAsync(&d->pstep, &step, 4, cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaMemsetAsync(&d->err, 0, sizeof(uint32_t), c->stream));  // a new state: an old capacity hit is history
     CU(c, cudaStreamSynchronize(c->stream));
     c->n_A = n32;
     c->kp_pending = false;  // A is new: nothing of the last P2 may be replayed
@@ -878,7 +986,7 @@ AXG_API int axg_step(axg_ctx* c, uint32_t n) {
         graphed = enqueue_steps_graph(c, n);
     if (graphed >= 0) launches = (uint64_t)graphed;
     else
-        for (uint32_t i = 0; i < n; ++i) launches += enqueue_phases(c, AXG_PHASE_ALL, prof, overlap);
+        for (uint32_t i = 0; i < n; ++i) launches += enqueue_phases(c, AXG_PHASE_ALL | AXG_PHASE_CONNECT, prof, overlap);
     if (c->adv_pending) {  // join: the ctx stream waits for the last step's cones
         CU(c, cudaStreamWaitEvent(c->stream, c->ev_adv, 0));
         c->adv_pending = false;
@@ -897,12 +1005,7 @@ AXG_API int axg_step(axg_ctx* c, uint32_t n) {
     c->last_launches = launches;
     c->last_particle_steps = h.particle_steps - ps0;
     c->n_A = c->n_B = h.n_live;
-    if (h.err) {
-        char msg[96];
-        std::snprintf(msg, sizeof msg, "device error word 0x%x (1 = particle capacity, 2 = polyline capacity)", h.err);
-        return fail(c, AXG_ECAPACITY, msg);
-    }
-    return AXG_OK;
+    return report_dev_err(c, h);
 }
 
 AXG_API int axg_check_capacity(axg_ctx* c, uint32_t n) {
@@ -918,12 +1021,34 @@ AXG_API int axg_check_capacity(axg_ctx* c, uint32_t n) {
 }
 
 AXG_API int axg_enqueue_phase(axg_ctx* c, uint32_t mask) {
-    if (!c || (mask & ~(uint32_t)AXG_PHASE_ALL)) return fail(c, AXG_EINVAL, "bad phase mask");
+    if (!c || (mask & ~(uint32_t)(AXG_PHASE_ALL | AXG_PHASE_CONNECT))) return fail(c, AXG_EINVAL, "bad phase mask");
     int rc = ensure_particles(c);
     if (rc) return rc;
     Prof prof{c, false};
     c->last_launches += (uint64_t)enqueue_phases(c, mask, prof);
     c->stepped = true;
+    return AXG_OK;
+}
+
+AXG_API int axg_enqueue_phase_on(axg_ctx* c, uint32_t mask, void* stream, int overlapped) {
+    if (!c || (mask & ~(uint32_t)(AXG_PHASE_ALL | AXG_PHASE_CONNECT))) return fail(c, AXG_EINVAL, "bad phase mask");
+    int rc = ensure_particles(c);
+    if (rc) return rc;
+    Prof prof{c, false};
+    c->last_launches += (uint64_t)enqueue_phases(c, mask, prof, false, (cudaStream_t)stream, true, overlapped != 0);
+    c->stepped = true;
+    return AXG_OK;
+}
+
+// FNV-1a over the kernel parameter block: everything a captured launch bakes in (pointers, sizes, modes)
+AXG_API int axg_params_fingerprint(axg_ctx* c, uint64_t* fp) {
+    if (!c || !fp) return AXG_EINVAL;
+    const int rc = ensure_particles(c);
+    if (rc) return rc;
+    uint64_t h = 1469598103934665603ull;
+    const unsigned char* b = reinterpret_cast<const unsigned char*>(&c->P);
+    for (size_t i = 0; i < sizeof(AxgParams); ++i) h = (h ^ b[i]) * 1099511628211ull;
+    *fp = h;
     return AXG_OK;
 }
 
@@ -937,12 +1062,11 @@ AXG_API int axg_sync(axg_ctx* c) {
     if (rc) return rc;
     c->n_A = c->n_B = h.n_live;
     c->last_particle_steps = h.particle_steps - c->ps0;
-    if (h.err) return fail(c, AXG_ECAPACITY, "device error word set");
-    return AXG_OK;
+    return report_dev_err(c, h);
 }
 
 AXG_API int axg_step_phase(axg_ctx* c, uint32_t mask) {
-    if (!c || (mask & ~(uint32_t)AXG_PHASE_ALL)) return fail(c, AXG_EINVAL, "bad phase mask");
+    if (!c || (mask & ~(uint32_t)(AXG_PHASE_ALL | AXG_PHASE_CONNECT))) return fail(c, AXG_EINVAL, "bad phase mask");
     int rc = ensure_particles(c);
     if (rc) return rc;
     AxgDev h;
@@ -957,8 +1081,7 @@ AXG_API int axg_step_phase(axg_ctx* c, uint32_t mask) {
     if (rc) return rc;
     if (mask & AXG_PHASE_DIFFUSE) c->n_B = h.n_live;
     if (mask & AXG_PHASE_BIN) c->n_A = c->n_B = h.n_live;
-    if (h.err) return fail(c, AXG_ECAPACITY, "device error word set");
-    return AXG_OK;
+    return report_dev_err(c, h);
 }
 
 namespace {
@@ -1004,17 +1127,17 @@ AXG_API int axg_read_state(axg_ctx* c, uint32_t field, void* dst, size_t dst_byt
     const size_t nA = have_p ? c->n_A : 0, nB = have_p ? c->n_B : 0, C = c->n_cones;
     switch (field) {
         case AXG_COUNTERS: {
-            if (n_elems) *n_elems = 8;
+            if (n_elems) *n_elems = 9;
             if (dst == nullptr && dst_bytes == 0) return AXG_OK;
-            if (dst == nullptr || dst_bytes < 64) return fail(c, AXG_ESMALL, "destination too small");
-            CU(c, cudaMemsetAsync(&((AxgDev*)c->d_dev)->cone_census[0], 0, 4 * sizeof(uint32_t), c->stream));
+            if (dst == nullptr || dst_bytes < 72) return fail(c, AXG_ESMALL, "destination too small");
+            CU(c, cudaMemsetAsync(&((AxgDev*)c->d_dev)->cone_census[0], 0, 5 * sizeof(uint32_t), c->stream));
             axg_launch_census(P, c->stream);
             AxgDev h;
             rc = read_dev(c, &h);
             if (rc) return rc;
-            const uint64_t v[8] = {h.step, h.n_live, h.next_id, h.emitted, h.absorbed,
-                                   h.cone_census[0], h.cone_census[1], h.cone_census[2]};
-            std::memcpy(dst, v, 64);
+            const uint64_t v[9] = {h.step, h.n_live, h.next_id, h.emitted, h.absorbed,
+                                   h.cone_census[0], h.cone_census[1], h.cone_census[2], h.n_connected};
+            std::memcpy(dst, v, 72);
             return AXG_OK;
         }
         case AXG_PART_X: return copy_out(c, P.A.x, nA, 4, dst, dst_bytes, n_elems);
@@ -1066,8 +1189,123 @@ AXG_API int axg_read_state(axg_ctx* c, uint32_t field, void* dst, size_t dst_byt
         case AXG_PRE_KEY:
             return export_out(c, nB, 4, dst, dst_bytes, n_elems,
                               [&](void* t) { axg_launch_pre_export(P, 4, c->b_chunked ? 1 : 0, t, c->stream); });
+        case AXG_CONE_TARGET: return copy_out(c, P.cone_target, C, 4, dst, dst_bytes, n_elems);
+        case AXG_GRAPH_VA:
+            return copy_out(c, c->G.Va, c->graph_built ? C + 1 : 0, 4, dst, dst_bytes, n_elems);
+        case AXG_GRAPH_EA:
+            return copy_out(c, c->G.Ea, c->graph_built ? c->graph_edges : 0, 4, dst, dst_bytes, n_elems);
+        case AXG_BFS_LEVEL:
+            return copy_out(c, c->G.C, c->bfs_done ? C : 0, 4, dst, dst_bytes, n_elems);
         default: return fail(c, AXG_EINVAL, "unknown field");
     }
+}
+
+// ---- connection formation, adjacency list, BFS (readings A-28..A-30) -------------------
+namespace {
+
+// the soma grid: cubic cells of 2^shift unit cells, edge >= reach, at most 2^21 cells; built once (somata do not move)
+int ensure_soma_grid(axg_ctx* c) {
+    if (c->soma_grid_built || c->n_cones == 0 || !(c->P.conn_thr > 0.0f)) return AXG_OK;
+    const float reach = c->r_cone + c->r_soma;
+    uint32_t shift = 0;
+    while ((float)(1u << shift) < reach) ++shift;
+    auto dim = [&](uint32_t n) { return (n + (1u << shift) - 1u) >> shift; };
+    while ((uint64_t)dim(c->grid.nx) * dim(c->grid.ny) * dim(c->grid.nz) > (1ull << 21)) ++shift;
+    const uint32_t gx = dim(c->grid.nx), gy = dim(c->grid.ny), gz = dim(c->grid.nz), cells = gx * gy * gz;
+    free_connect(c);
+    void* ptr[4];
+    const size_t sizes[4] = {((size_t)cells + 1) * 4, ((size_t)cells + 1) * 4, ((size_t)cells + 1) * 4, (size_t)c->n_cones * 4};
+    for (int i = 0; i < 4; ++i) {
+        ptr[i] = dev_alloc(c, sizes[i]);
+        if (!ptr[i]) return fail(c, AXG_ECUDA, "device allocation failed (soma grid)");
+        c->connect_bufs.push_back(ptr[i]);
+    }
+    c->P.ng_shift = shift; c->P.ngx = gx; c->P.ngy = gy; c->P.ngz = gz;
+    c->P.ng_lo = (const uint32_t*)ptr[2];
+    c->P.ng_list = (const uint32_t*)ptr[3];
+    axg_launch_soma_grid(c->P, (uint32_t*)ptr[0], (uint32_t*)ptr[1], (uint32_t*)ptr[2], (uint32_t*)ptr[3], cells, c->stream);
+    c->soma_grid_built = true;
+    return after_sync(c, "soma grid");
+}
+
+int ensure_graph_bufs(axg_ctx* c) {
+    if (!c->graph_bufs.empty()) return AXG_OK;
+    const size_t n = c->n_cones;
+    const size_t sizes[] = {(n + 1) * 4, (n + 1) * 4, (n + 1) * 4, n * 4 + 4, n * 4 + 4, (n / 33 + 2) * 4, 4, (n + 1) * 4,
+                            2 * n * 4 + 4, n * 4 + 4, n + 4, n + 4, n + 4, 4};
+    constexpr int NB = 14;
+    void* ptr[NB];
+    for (int i = 0; i < NB; ++i) {
+        ptr[i] = dev_alloc(c, sizes[i]);
+        if (!ptr[i]) return fail(c, AXG_ECUDA, "device allocation failed (graph)");
+        c->graph_bufs.push_back(ptr[i]);
+    }
+    AxgGraph& g = c->G;
+    g.n = (uint32_t)n;
+    g.cnt = (uint32_t*)ptr[0]; g.cursor = (uint32_t*)ptr[1]; g.in_lo = (uint32_t*)ptr[2]; g.in_list = (uint32_t*)ptr[3];
+    g.scratch = (uint32_t*)ptr[4]; g.big = (uint32_t*)ptr[5]; g.n_big = (uint32_t*)ptr[6]; g.Va = (uint32_t*)ptr[7];
+    g.Ea = (uint32_t*)ptr[8]; g.C = (int32_t*)ptr[9]; g.F = (uint8_t*)ptr[10]; g.Fu = (uint8_t*)ptr[11];
+    g.X = (uint8_t*)ptr[12]; g.flag = (uint32_t*)ptr[13];
+    return AXG_OK;
+}
+
+}  // namespace
+
+AXG_API int axg_set_connect(axg_ctx* c, float r_cone, float r_soma) {
+    if (!c || !(r_cone >= 0.0f) || !(r_soma >= 0.0f) || !std::isfinite(r_cone) || !std::isfinite(r_soma) ||
+        r_cone + r_soma > 64.0f)
+        return fail(c, AXG_EINVAL, "bad radii");
+    const float reach = r_cone + r_soma;
+    c->r_cone = r_cone; c->r_soma = r_soma;
+    c->P.conn_thr = reach > 0.0f ? reach * reach : 0.0f;
+    free_connect(c);  // the soma grid depends on the reach
+    return ensure_soma_grid(c);
+}
+
+AXG_API int axg_load_targets(axg_ctx* c, const uint32_t* target, uint32_t n) {
+    if (!c || (!target && n)) return fail(c, AXG_EINVAL, "null argument");
+    if (n != c->n_cones) return fail(c, AXG_EINVAL, "cone count differs from the placed count");
+    for (uint32_t i = 0; i < n; ++i)
+        if (target[i] != 0xffffffffu && (target[i] >= n || target[i] == i)) return fail(c, AXG_EINVAL, "bad target");
+    if (n) CU(c, cudaMemcpyAsync(c->P.cone_target, target, (size_t)n * 4, cudaMemcpyHostToDevice, c->stream));
+    c->graph_built = c->bfs_done = false;
+    return after_sync(c, "axg_load_targets");
+}
+
+AXG_API int axg_build_graph(axg_ctx* c, int directed) {
+    if (!c) return AXG_EINVAL;
+    c->graph_built = c->bfs_done = false;
+    c->graph_edges = 0;
+    if (c->n_cones == 0) return fail(c, AXG_ESTATE, "no neurons placed");
+    int rc = ensure_graph_bufs(c);
+    if (rc) return rc;
+    c->G.directed = directed ? 1 : 0;
+    c->G.target = c->P.cone_target;
+    axg_launch_graph_build(c->G, c->stream);
+    CU(c, cudaMemcpyAsync(&c->graph_edges, c->G.Va + c->n_cones, 4, cudaMemcpyDeviceToHost, c->stream));
+    rc = after_sync(c, "axg_build_graph");
+    if (rc) return rc;
+    c->graph_built = true;
+    return AXG_OK;
+}
+
+AXG_API int axg_bfs(axg_ctx* c, uint32_t root) {
+    if (!c) return AXG_EINVAL;
+    if (!c->graph_built) return fail(c, AXG_ESTATE, "no graph: call axg_build_graph first");
+    if (root >= c->n_cones) return fail(c, AXG_EINVAL, "root out of range");
+    c->bfs_done = false;
+    axg_launch_bfs_init(c->G, root, c->stream);
+    for (uint32_t level = 0; level <= c->n_cones; ++level) {   // "repeated until frontier is empty"
+        uint32_t more = 0;
+        CU(c, cudaMemsetAsync(c->G.flag, 0, 4, c->stream));
+        axg_launch_bfs_level(c->G, c->stream);
+        CU(c, cudaMemcpyAsync(&more, c->G.flag, 4, cudaMemcpyDeviceToHost, c->stream));
+        const int rc = after_sync(c, "axg_bfs");
+        if (rc) return rc;
+        if (!more) break;
+    }
+    c->bfs_done = true;
+    return AXG_OK;
 }
 
 AXG_API int axg_sense_buffer(axg_ctx* c, void** device_ptr, size_t* bytes) {

@@ -193,8 +193,8 @@ __global__ void k_pre_export(const AxgParams p, int component, int chunked, void
         if (chunked && axg_is_hole(p, o, n_phys)) continue;
         const uint32_t i = chunked ? axg_dense_index(p, o, n_phys, n_surv) : o;
         if (component < 4) static_cast<uint32_t*>(dst)[i] = rec[(size_t)o * 4 + component];
-        else if (component == 4) static_cast<uint32_t*>(dst)[i] = p.key_pre[o];
-        else static_cast<uint8_t*>(dst)[i] = chunked ? (uint8_t)(p.arr_pre[o] >> 30) : p.Bsp[o];
+        else if (component == 4) static_cast<uint32_t*>(dst)[i] = chunked ? p.kw[o].x : p.key_pre[o];
+        else static_cast<uint8_t*>(dst)[i] = chunked ? (uint8_t)(p.kw[o].y >> 30) : p.Bsp[o];
     }
 }
 // the permutation (sorted slot -> pre-sort index) without the species bits

@@ -117,8 +117,10 @@ __global__ void __launch_bounds__(256) k_sense_particles(const AxgParams p) {
         for (int s = 0; s < AXG_MAX_SPECIES_D; ++s)
 #pragma unroll
             for (int a = 0; a < 4; ++a) acc[s][a] = 0;
-        // bricked cell order: the x range of a row crosses at most max_seg bricks, one contiguous run in each
-        const int max_seg = p.key_order ? ((2 * (int)ceilf(Rm) + 8) >> 3) + 1 : 1;
+        // bricked cell order: the x range of a row crosses at most max_seg bricks, one contiguous run in each (Z-order:
+        // runs of two cells -- x bit 0 is key bit 0)
+        const int seg_shift = p.key_order == 1 ? 3 : 1;
+        const int max_seg = p.key_order ? ((2 * (int)ceilf(Rm) + (1 << seg_shift)) >> seg_shift) + 1 : 1;
         for (int r0 = 0; r0 < n_rows; r0 += 32)
         for (int seg = 0; seg < max_seg; ++seg) {
             const int r = r0 + lane;
@@ -132,10 +134,10 @@ __global__ void __launch_bounds__(256) k_sense_particles(const AxgParams p) {
                 if (left >= 0.0f) {
                     const float hw = sqrtf(left) * 1.00001f + 1e-5f;
                     int x0 = max(0, (int)floorf(qx - hw)), x1 = min((int)p.nx - 1, (int)floorf(qx + hw));
-                    if (p.key_order) {  // the seg-th brick of the range
-                        const int bx = (x0 >> 3) + seg;
-                        x0 = max(x0, bx << 3);
-                        x1 = min(x1, (bx << 3) + 7);
+                    if (p.key_order) {  // the seg-th brick (run) of the range
+                        const int bx = (x0 >> seg_shift) + seg;
+                        x0 = max(x0, bx << seg_shift);
+                        x1 = min(x1, (bx << seg_shift) + (1 << seg_shift) - 1);
                     }
                     if (x1 >= x0) {
                         a = __ldg(cell_lo + axg_key_of_cell(p, (uint32_t)x0, (uint32_t)y, (uint32_t)z));
@@ -290,6 +292,7 @@ __global__ void k_census(const AxgParams p) {
     for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < p.n_cones; c += gridDim.x * blockDim.x) {
         const uint32_t st = p.cone_state[c];
         if (st < 3u) atomicAdd(&s_c[st], 1u);
+        if (st == 3u) atomicAdd(&p.dev->n_connected, 1u);  // connection formation only: rare
         if (st == 0u) atomicMax(&s_c[3], p.poly_len[c]);  // longest ACTIVE polyline (capacity pre-check)
     }
     __syncthreads();

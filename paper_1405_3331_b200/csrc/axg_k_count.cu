@@ -32,6 +32,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) k_cell_scan(const AxgParams p) {
     const uint32_t n_el = p.cells + 1u;  // cell_lo[cells] = n_live
     const uint32_t n_tiles = (n_el + AXG_SCAN_TILE - 1) / AXG_SCAN_TILE;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (blockIdx.x == 0 && tid == 0) dev->n_big = 0u;  // the list of crowded cells that k_place builds for k_settle
 
     while (true) {
         __syncthreads();
@@ -119,6 +120,7 @@ __global__ void __launch_bounds__(SCAN_THREADS, SCAN2_BLOCKS_PER_SM) k_cell_scan
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t G = gridDim.x, b = blockIdx.x;
     const uint32_t gen = *(volatile uint32_t*)&dev->epoch;  // read before this block arrives at the barrier
+    if (b == 0 && tid == 0) dev->n_big = 0u;  // the list of crowded cells that k_place builds for k_settle
     const uint32_t n_el = p.cells + 1u;
     const uint32_t n_tiles = (n_el + AXG_SCAN_TILE - 1) / AXG_SCAN_TILE;
     const uint32_t per = (n_tiles + G - 1u) / G;
@@ -216,6 +218,13 @@ __global__ void __launch_bounds__(SCAN_THREADS, SCAN2_BLOCKS_PER_SM) k_cell_scan
 
 // ---- slot[cell start + arrival rank] = pre-sort row | species << 30 ---------------------------------------------------------
 constexpr int PLACE_THREADS = 256;
+// Cells with more members than this are not ranked member by member (a loop over the cell per member: quadratic in the
+// occupancy) but as a whole, by one block (settle_big_cell below).  k_place lists them: the row whose arrival rank is
+// exactly SETTLE_INLINE exists once in every cell with more than SETTLE_INLINE members.
+constexpr uint32_t SETTLE_INLINE = 32u;
+#ifndef AXG_PLACE_PREFETCH
+#define AXG_PLACE_PREFETCH 1
+#endif
 
 __global__ void __launch_bounds__(PLACE_THREADS) k_place(const AxgParams p) {
     // B is in the chunked layout of k_diffuse_chunked: every physical row below n_pp is visited, the holes at the end
@@ -225,12 +234,37 @@ __global__ void __launch_bounds__(PLACE_THREADS) k_place(const AxgParams p) {
     const uint32_t* __restrict__ cell_lo = p.cell_lo;
     // one particle per thread: the kernel is bound by L2 transactions (one random 4-byte read of the cell start + one
     // scattered 4-byte store each) and wants many warps in flight.  No atomic: the counting atomic of P1 already
-    // returned every row's arrival rank inside its cell (arr_pre), in the arbitrary order of the atomics.
+    // returned every row's arrival rank inside its cell (kw.y), in the arbitrary order of the atomics.
+#if AXG_PLACE_PREFETCH
+    // the first touch of a sector of cell_lo is a random read at DRAM latency: sweep cell_lo into the L2 one grid sweep
+    // (+ the reach of a particle's move) ahead, as k_diffuse_chunked does for cnt
+    uint32_t pf_prev = 0xffffffffu;
+    const uint32_t pf_reach = (uint32_t)min((float)p.cells, (6.0f * p.sigma + 1.5f) * (p.key_order == 0 ? (float)p.nx * (float)p.ny
+                                                                                                : 4096.0f));
+#endif
     for (uint32_t o = blockIdx.x * PLACE_THREADS + threadIdx.x; o < n_pp; o += gridDim.x * PLACE_THREADS) {
+#if AXG_PLACE_PREFETCH
+        {   // warp-uniform: every lane of the warp is inside the loop (n_pp is padded by the grid-stride test below)
+            const uint32_t act = __activemask();
+            const uint32_t kk = __ldg(&p.kw[o].x);
+            const int leader = __ffs(act) - 1, last = 31 - __clz(act);
+            const uint32_t k0 = __shfl_sync(act, kk, leader), k1 = __shfl_sync(act, kk, last);
+            if ((threadIdx.x & 31) == leader) {
+                // keys of a chunk's survivors are those of neighbouring input rows +- the move: take the span generously
+                if (pf_prev != 0xffffffffu && k0 > pf_prev) {
+                    const unsigned long long lo = (unsigned long long)k0 + (k0 - pf_prev) + pf_reach;
+                    if (lo + 64ull < p.cells) axg_prefetch_l2(cell_lo + (lo & ~3ull), 256u);
+                }
+                pf_prev = k0;
+            }
+            (void)k1;
+        }
+#endif
         if (o < n_phys && (o % AXG_CHUNK) >= __ldg(p.chunk_cnt + o / AXG_CHUNK)) continue;  // a hole
-        const uint32_t k = __ldg(p.key_pre + o);
-        const uint32_t a = __ldg(p.arr_pre + o);  // arrival rank | species << 30
-        slot[__ldg(cell_lo + k) + (a & AXG_IDX_MASK)] = o | (a & ~AXG_IDX_MASK);
+        const uint2 w = __ldg(p.kw + o);  // key, arrival rank | species << 30: one 8-byte load
+        const uint32_t arr = w.y & AXG_IDX_MASK;
+        slot[__ldg(cell_lo + w.x) + arr] = o | (w.y & ~AXG_IDX_MASK);
+        if (arr == SETTLE_INLINE) p.big_list[atomicAdd(&p.dev->n_big, 1u)] = w.x;  // at most n_live / 33 entries
     }
 }
 
@@ -239,25 +273,158 @@ constexpr int SETTLE_THREADS = 256;
 constexpr int SETTLE_ITEMS = 1;  // warp-striped (item i of lane l is slot base + 32 i + l).  Measured at C3: 1 item and
                                  // 8 blocks per SM 0.188 ms, 2 items 0.198, 4 items / 6 blocks 0.227, 8 items 0.272 --
                                  // the kernel lives on many independent warps in flight, not on ILP inside one
+#ifndef AXG_SETTLE_SORT_MAX
+#define AXG_SETTLE_SORT_MAX 1024
+#endif
+constexpr uint32_t SETTLE_SORT_MAX = AXG_SETTLE_SORT_MAX;
+#ifndef AXG_SETTLE_PREFETCH
+#define AXG_SETTLE_PREFETCH 5   // look-ahead of the record prefetch in half grid sweeps (0 = off)
+#endif  // members of a cell that one block sorts in shared memory
+
+template <bool WITH_KP>
+__device__ __forceinline__ void settle_store(const AxgParams& p, uint32_t dst, const float4& r, uint32_t v, uint32_t k) {
+    p.A.x[dst] = r.x;
+    p.A.y[dst] = r.y;
+    p.A.z[dst] = r.z;
+    p.A.id[dst] = __float_as_uint(r.w);
+    p.A.species[dst] = (uint8_t)(v >> 30);
+    if (WITH_KP) {
+        p.skey[p.final_buf][dst] = k;
+        p.sidx[p.final_buf][dst] = v;
+    }
+}
+
+// One block puts ONE crowded cell (more than SETTLE_INLINE members) into pre-sort order.
+//  m <= SETTLE_SORT_MAX: the members' slot values are sorted in shared memory (bitonic network: O(m log^2 m)), then
+//     gathered in that order.
+//  larger: the members are the valid rows with this key among the physical rows [min, max] of its slot list, and a
+//     row's rank is the number of such rows before it: one pass over that window with a running count (O(window); the
+//     window of a cell is the neighbourhood its particles came from -- the whole array in the worst case).
+// Either way the cost per member no longer grows with the occupancy (D = 0 piles a source's whole emission into one
+// cell: SURVEY.md §8(a) P2b-P2d, reading A-9).
+template <bool WITH_KP>
+__device__ void settle_big_cell(const AxgParams& p, uint32_t key, uint32_t* s_sort, uint32_t* s_scan) {
+    const uint32_t* __restrict__ slot = p.sidx[p.final_buf ^ 1];
+    const uint32_t lo = p.cell_lo[key], hi = p.cell_lo[key + 1u], m = hi - lo;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (m <= SETTLE_SORT_MAX) {
+        uint32_t n2 = 64u;
+        while (n2 < m) n2 <<= 1;
+        // rotate the value left by two: index in the top 30 bits, species in the low 2 -> integer order = index order
+        for (uint32_t i = tid; i < n2; i += SETTLE_THREADS) {
+            const uint32_t v = i < m ? slot[lo + i] : 0xffffffffu;
+            s_sort[i] = i < m ? ((v << 2) | (v >> 30)) : 0xffffffffu;
+        }
+        __syncthreads();
+        for (uint32_t size = 2u; size <= n2; size <<= 1)
+            for (uint32_t stride = size >> 1; stride > 0u; stride >>= 1) {
+                for (uint32_t t = tid; t < (n2 >> 1); t += SETTLE_THREADS) {
+                    const uint32_t i = 2u * t - (t & (stride - 1u)), j = i + stride;
+                    const uint32_t a = s_sort[i], b = s_sort[j];
+                    const bool up = (i & size) == 0u;
+                    if ((a > b) == up) { s_sort[i] = b; s_sort[j] = a; }
+                }
+                __syncthreads();
+            }
+        for (uint32_t i = tid; i < m; i += SETTLE_THREADS) {
+            const uint32_t w = s_sort[i], v = (w >> 2) | (w << 30);
+            settle_store<WITH_KP>(p, lo + i, p.Brec[v & AXG_IDX_MASK], v, key);
+        }
+        __syncthreads();
+        return;
+    }
+    // ---- the window of physical rows that holds the members ----
+    uint32_t pmin = 0xffffffffu, pmax = 0u;
+    for (uint32_t i = tid; i < m; i += SETTLE_THREADS) {
+        const uint32_t o = slot[lo + i] & AXG_IDX_MASK;
+        pmin = min(pmin, o);
+        pmax = max(pmax, o);
+    }
+    pmin = __reduce_min_sync(0xffffffffu, pmin);
+    pmax = __reduce_max_sync(0xffffffffu, pmax);
+    if (lane == 0) { s_scan[warp] = pmin; s_scan[8 + warp] = pmax; }
+    __syncthreads();
+    for (int w = 0; w < SETTLE_THREADS / 32; ++w) { pmin = min(pmin, s_scan[w]); pmax = max(pmax, s_scan[8 + w]); }
+    __syncthreads();
+    const uint32_t n_phys = p.dev->n_phys;
+    uint32_t running = 0u;
+    constexpr uint32_t PER = 4u, TILE = SETTLE_THREADS * PER;  // four consecutive rows per thread
+    for (uint32_t t0 = pmin; t0 <= pmax && t0 >= pmin; t0 += TILE) {
+        const uint32_t first = t0 + tid * PER;
+        uint2 w[PER];
+        uint32_t mine = 0u, flags = 0u;
+#pragma unroll
+        for (uint32_t q = 0; q < PER; ++q) {
+            const uint32_t o = first + q;
+            bool ok = o <= pmax && o >= first;
+            if (ok && o < n_phys) ok = (o % AXG_CHUNK) < p.chunk_cnt[o / AXG_CHUNK];  // not a hole (stale words)
+            w[q] = ok ? p.kw[o] : make_uint2(0u, 0u);
+            ok = ok && w[q].x == key;
+            flags |= ok ? (1u << q) : 0u;
+            mine += ok ? 1u : 0u;
+        }
+        uint32_t incl = mine;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t u = __shfl_up_sync(0xffffffffu, incl, d);
+            if (lane >= d) incl += u;
+        }
+        if (lane == 31) s_scan[warp] = incl;
+        __syncthreads();
+        uint32_t before = running, total = 0u;
+        for (int ww = 0; ww < SETTLE_THREADS / 32; ++ww) {
+            const uint32_t c = s_scan[ww];
+            before += ww < warp ? c : 0u;
+            total += c;
+        }
+        uint32_t dst = lo + before + incl - mine;
+#pragma unroll
+        for (uint32_t q = 0; q < PER; ++q)
+            if ((flags >> q) & 1u) {
+                const uint32_t o = first + q;
+                settle_store<WITH_KP>(p, dst++, p.Brec[o], o | (w[q].y & ~AXG_IDX_MASK), key);
+            }
+        running += total;
+        __syncthreads();
+    }
+}
 
 // WITH_KP: also store the sorted keys and the permutation.  Nothing on the path reads them (P1 recomputes the key, P3
 // works from cell_lo), so the step runs the lean kernel and axg_read_state(AXG_KEYS_SORTED / AXG_PERM) replays the
 // full one on the intact inputs (slot list, records, cell_lo): the same values land in the same places.
 template <bool WITH_KP>
 __global__ void __launch_bounds__(SETTLE_THREADS, 8) k_settle(const AxgParams p) {
+    __shared__ uint32_t s_sort[SETTLE_SORT_MAX];
+    __shared__ uint32_t s_scan[16];
     const uint32_t n = p.dev->n_live;
     const uint32_t* __restrict__ slot = p.sidx[p.final_buf ^ 1];
-    uint32_t* __restrict__ perm = p.sidx[p.final_buf];
-    uint32_t* __restrict__ keys = p.skey[p.final_buf];
     const float4* __restrict__ rec = p.Brec;
     const uint32_t* __restrict__ cell_lo = p.cell_lo;
     const int lane = threadIdx.x & 31;
     const uint32_t warps_total = (gridDim.x * SETTLE_THREADS) >> 5;
     const uint32_t chunk = 32u * SETTLE_ITEMS;
+#if AXG_SETTLE_PREFETCH
+    // The record gather is the one access of this kernel that misses the L2: a slot's record sits within a few cell
+    // planes of the slot's own index in the pre-sort array (a particle moves a few cells per step), and every 32-byte
+    // sector of that array is first touched by a random 16-byte read, i.e. at DRAM latency.  So the array is swept into
+    // the L2 sequentially, AXG_SETTLE_PREFETCH / 2 grid sweeps ahead of the gathers (one 512-byte bulk prefetch per warp
+    // trip), and the gathers hit.
+    const uint32_t n_pp = p.dev->n_pp;
+    const uint32_t look = (warps_total * chunk / 2u) * AXG_SETTLE_PREFETCH;
+#endif
     for (uint32_t base = ((blockIdx.x * SETTLE_THREADS + threadIdx.x) >> 5) * chunk; base < n;
          base += warps_total * chunk) {
         uint32_t v[SETTLE_ITEMS];
         float4 r[SETTLE_ITEMS];
+#if AXG_SETTLE_PREFETCH
+        if (lane == 0) {
+            const uint32_t row = base + look;
+            if (row + chunk <= n_pp) axg_prefetch_l2(rec + row, chunk * (uint32_t)sizeof(float4));
+            if (base < warps_total * chunk && look > warps_total * chunk)   // first sweep: also what lies before `look`
+                for (uint32_t q = base + warps_total * chunk; q < look + base && q + chunk <= n_pp; q += warps_total * chunk)
+                    axg_prefetch_l2(rec + q, chunk * (uint32_t)sizeof(float4));
+        }
+#endif
 #pragma unroll
         for (int i = 0; i < SETTLE_ITEMS; ++i) {
             const uint32_t j = base + 32u * i + lane;
@@ -275,21 +442,16 @@ __global__ void __launch_bounds__(SETTLE_THREADS, 8) k_settle(const AxgParams p)
             const uint32_t idx = v[i] & AXG_IDX_MASK;
             const uint32_t k = axg_cell_key(p, r[i].x, r[i].y, r[i].z);
             const uint32_t lo = __ldg(cell_lo + k), hi = __ldg(cell_lo + k + 1u);
+            if (hi - lo > SETTLE_INLINE) continue;  // a crowded cell: settle_big_cell below
             uint32_t rank = 0u;  // members of my cell with a smaller pre-sort index (reading A-9: ties keep that order)
             if (hi - lo > 1u)  // alone in the cell (the common case): nothing to rank against
                 for (uint32_t q = lo; q < hi; ++q) rank += ((__ldg(slot + q) & AXG_IDX_MASK) < idx) ? 1u : 0u;
-            const uint32_t dst = lo + rank;
-            p.A.x[dst] = r[i].x;
-            p.A.y[dst] = r[i].y;
-            p.A.z[dst] = r[i].z;
-            p.A.id[dst] = __float_as_uint(r[i].w);
-            p.A.species[dst] = (uint8_t)(v[i] >> 30);
-            if (WITH_KP) {
-                keys[dst] = k;
-                perm[dst] = v[i];
-            }
+            settle_store<WITH_KP>(p, lo + rank, r[i], v[i], k);
         }
     }
+    // the crowded cells that k_place listed (a few hundred at C3..C5: the cells next to a source), one block each
+    const uint32_t n_big = p.dev->n_big;
+    for (uint32_t w = blockIdx.x; w < n_big; w += gridDim.x) settle_big_cell<WITH_KP>(p, p.big_list[w], s_sort, s_scan);
 }
 
 }  // namespace

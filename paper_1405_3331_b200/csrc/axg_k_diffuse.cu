@@ -22,7 +22,7 @@ __device__ __forceinline__ void tally(const AxgParams& p, uint32_t (*s_hist)[AXG
                                       uint32_t species) {
     if (p.bin_mode == AXG_BIN_COUNT_D) {
         // the old count = this row's arrival rank inside its cell; the species rides in its top two bits (no Bsp column)
-        p.arr_pre[o] = atomicAdd(p.cnt + key, 1u) | (species << 30);
+        p.kw[o] = make_uint2(key, atomicAdd(p.cnt + key, 1u) | (species << 30));
     } else {
 #pragma unroll
         for (int q = 0; q < AXG_MAX_PASSES; ++q)
@@ -64,8 +64,8 @@ __device__ void emit_and_close(const AxgParams& p, int do_emit, uint32_t (*s_his
             const uint32_t key = axg_cell_key(p, sd.x, sd.y, sd.z);
             p.Brec[o] = make_float4(sd.x, sd.y, sd.z, __uint_as_float(next_id + p.src_id_prefix[s] + j));
             if (p.bin_mode != AXG_BIN_COUNT_D) p.Bsp[o] = (uint8_t)(sd.species_polarity & 0xffu);
-            p.key_pre[o] = key;
             if (p.bin_mode != AXG_BIN_COUNT_D) {
+                p.key_pre[o] = key;
                 tally(p, s_hist, key, o, 0u);
             } else if (j == 0u) {  // all newborns of a source share its cell: one atomic per source, not per particle
                 p.src_arr[s] = atomicAdd(p.cnt + key, p.src_emit_prefix[s + 1] - p.src_emit_prefix[s]);
@@ -80,7 +80,9 @@ __device__ void emit_and_close(const AxgParams& p, int do_emit, uint32_t (*s_his
                 const uint32_t mid = (lo + hi) >> 1;
                 if (p.src_emit_prefix[mid] <= e) lo = mid; else hi = mid;
             }
-            p.arr_pre[n_phys + e] = (p.src_arr[lo] + (e - p.src_emit_prefix[lo])) | ((p.src[lo].species_polarity & 0xffu) << 30);
+            const AxgSourceDev sd = p.src[lo];
+            p.kw[n_phys + e] = make_uint2(axg_cell_key(p, sd.x, sd.y, sd.z),
+                                          (p.src_arr[lo] + (e - p.src_emit_prefix[lo])) | ((sd.species_polarity & 0xffu) << 30));
         }
     }
     if (p.bin_mode != AXG_BIN_COUNT_D) {
@@ -284,8 +286,26 @@ __global__ void __launch_bounds__(DIFF_THREADS, 4) k_diffuse(const AxgParams p) 
 #ifndef AXG_CHUNKED_BLOCKS
 #define AXG_CHUNKED_BLOCKS 4
 #endif
+#ifndef AXG_P1_DEFER
+#define AXG_P1_DEFER 1    // store a chunk's {key, arrival rank} words one trip later (the atomics' round trip is hidden)
+#endif
+#ifndef AXG_P1_PREFETCH
+#define AXG_P1_PREFETCH 1  // sweep the count array into the L2 ahead of the counting atomics (see the kernel)
+#endif
+#ifndef AXG_P1_STAGES
+#define AXG_P1_STAGES 2   // chunks in flight per warp (bulk-async staging); 0 = per-lane loads held in registers
+#endif
+// One stage = the five column runs of one chunk: x, y, z, id (512 B each) and species (128 B).  A chunk column is one
+// 16-byte-aligned run of global memory, so each is ONE 1-D bulk copy (cp.async.bulk -> SASS UBLKCP) whose completion
+// is counted on the stage's mbarrier: the bytes in flight no longer sit in registers behind the scoreboard, and a warp
+// only ever waits for data that was requested two chunks ago.
+constexpr int P1_STAGE_BYTES = 4 * 512 + 128;
+constexpr int P1_SMEM = DIFF_WARPS * (AXG_P1_STAGES > 0 ? AXG_P1_STAGES : 1) * P1_STAGE_BYTES;
+static_assert(P1_SMEM >= (int)(AXG_MAX_PASSES * AXG_RADIX * sizeof(uint32_t)), "emit_and_close reuses the staging area");
+
 __global__ void __launch_bounds__(DIFF_THREADS, AXG_CHUNKED_BLOCKS) k_diffuse_chunked(const AxgParams p) {
-    __shared__ uint32_t s_hist[AXG_MAX_PASSES][AXG_RADIX];  // scratch of emit_and_close only
+    extern __shared__ __align__(128) unsigned char s_raw[];
+    __shared__ __align__(8) unsigned long long s_bar[DIFF_WARPS][AXG_P1_STAGES > 0 ? AXG_P1_STAGES : 1];
     __shared__ uint32_t s_surv;
     AxgDev* dev = p.dev;
     const uint32_t n_in = dev->n_live, t = dev->pstep;
@@ -295,14 +315,68 @@ __global__ void __launch_bounds__(DIFF_THREADS, AXG_CHUNKED_BLOCKS) k_diffuse_ch
     const AxgRoundKeys rk = axg_round_keys(p.seed_lo, p.seed_hi);
     static_assert(32 * DIFF_ITEMS == AXG_CHUNK, "one warp trip = one chunk");
     if (tid == 0) s_surv = 0u;
-    __syncthreads();
 
     uint32_t mine = 0u;  // survivors of my warp's chunks (lane 0)
     const uint32_t warps_total = (gridDim.x * DIFF_THREADS) >> 5;
-    for (uint32_t chunk = (blockIdx.x * DIFF_THREADS + tid) >> 5; chunk < n_chunks; chunk += warps_total) {
+    const uint32_t gw = (blockIdx.x * DIFF_THREADS + tid) >> 5;
+#if AXG_P1_STAGES > 0
+    unsigned char* const my_stage = s_raw + (size_t)(tid >> 5) * AXG_P1_STAGES * P1_STAGE_BYTES;
+    const uint32_t my_stage_u32 = axg_smem_u32(my_stage), my_bar_u32 = axg_smem_u32(&s_bar[tid >> 5][0]);
+    auto request = [&](uint32_t chunk, int st) {  // lane 0: arm the stage's barrier, then the five bulk copies
+        const uint32_t bar = my_bar_u32 + 8u * st, dst = my_stage_u32 + (uint32_t)st * P1_STAGE_BYTES;
+        const size_t r0 = (size_t)chunk * AXG_CHUNK;  // the arrays are padded: the last chunk may read past n_in
+        axg_mbar_expect_tx(bar, P1_STAGE_BYTES);
+        axg_bulk_g2s(dst, p.A.x + r0, 512u, bar);
+        axg_bulk_g2s(dst + 512u, p.A.y + r0, 512u, bar);
+        axg_bulk_g2s(dst + 1024u, p.A.z + r0, 512u, bar);
+        axg_bulk_g2s(dst + 1536u, p.A.id + r0, 512u, bar);
+        axg_bulk_g2s(dst + 2048u, p.A.species + r0, 128u, bar);
+    };
+    if (lane == 0) {
+#pragma unroll
+        for (int st = 0; st < AXG_P1_STAGES; ++st) axg_mbar_init(my_bar_u32 + 8u * st, 1u);
+        axg_fence_mbar_init();
+#pragma unroll
+        for (int st = 0; st < AXG_P1_STAGES; ++st)
+            if (gw + st * warps_total < n_chunks) request(gw + st * warps_total, st);
+    }
+    __syncwarp();
+    int st = 0;
+    uint32_t parity = 0u;
+#endif
+    __syncthreads();  // s_surv
+#if AXG_P1_PREFETCH
+    uint32_t pf_prev = 0xffffffffu;
+    // how far beyond its own cell a particle's counting atomic can land: 6 sigma in z (planes of nx ny cells; linear key)
+    const uint32_t pf_reach = (uint32_t)min((float)p.cells, (6.0f * p.sigma + 1.5f) * (p.key_order == 0 ? (float)p.nx * (float)p.ny
+                                                                                                : 4096.0f));
+#endif
+#if AXG_P1_DEFER
+    bool have_pend = false;
+    uint32_t palive = 0u, psp = 0u, pdst[DIFF_ITEMS], parr[DIFF_ITEMS], pkey[DIFF_ITEMS];
+#pragma unroll
+    for (int i = 0; i < DIFF_ITEMS; ++i) { pdst[i] = 0u; parr[i] = 0u; pkey[i] = 0u; }
+#endif
+
+    for (uint32_t chunk = gw; chunk < n_chunks; chunk += warps_total) {
         const uint32_t first = chunk * AXG_CHUNK + lane;
         float x[DIFF_ITEMS], y[DIFF_ITEMS], z[DIFF_ITEMS];
         uint32_t id[DIFF_ITEMS], sp[DIFF_ITEMS];
+#if AXG_P1_STAGES > 0
+        axg_mbar_wait(my_bar_u32 + 8u * st, parity);
+        {
+            const unsigned char* sb = my_stage + (size_t)st * P1_STAGE_BYTES;
+#pragma unroll
+            for (int i = 0; i < DIFF_ITEMS; ++i) {  // warp-striped rows, as in memory: conflict-free
+                const int r = i * 32 + lane;
+                x[i] = reinterpret_cast<const float*>(sb)[r];
+                y[i] = reinterpret_cast<const float*>(sb + 512)[r];
+                z[i] = reinterpret_cast<const float*>(sb + 1024)[r];
+                id[i] = reinterpret_cast<const uint32_t*>(sb + 1536)[r];
+                sp[i] = sb[2048 + r];
+            }
+        }
+#else
 #pragma unroll
         for (int i = 0; i < DIFF_ITEMS; ++i) {
             const uint32_t g = first + i * 32;
@@ -319,51 +393,119 @@ __global__ void __launch_bounds__(DIFF_THREADS, AXG_CHUNKED_BLOCKS) k_diffuse_ch
                 asm volatile("ld.global.nc.u8 %0, [%1];" : "=r"(sp[i]) : "l"(p.A.species + g) : "memory");
             }
         }
+#endif
+#if AXG_P1_PREFETCH
+        // A counting atomic on a sector of cnt that is not in the L2 waits for DRAM (one in eight: a sector holds eight
+        // cells and each cell gets about one particle).  All warps sweep the sorted input in step, so the keys that the
+        // NEXT trip of this warp will hit lie one sweep ahead of the keys of this trip, +- the few cell planes a particle
+        // moves: every warp asks for its own span of cnt, shifted by (one sweep + that reach), with one bulk L2 prefetch.
+        // The sweep length in keys is measured from the warp's own previous trip.
+        {
+            const uint32_t k_first = axg_cell_key(p, fmaxf(x[0], 0.0f), fmaxf(y[0], 0.0f), fmaxf(z[0], 0.0f));
+            const uint32_t k_last = axg_cell_key(p, fmaxf(x[DIFF_ITEMS - 1], 0.0f), fmaxf(y[DIFF_ITEMS - 1], 0.0f),
+                                                 fmaxf(z[DIFF_ITEMS - 1], 0.0f));
+            const uint32_t k0 = __shfl_sync(0xffffffffu, k_first, 0), k1 = __shfl_sync(0xffffffffu, k_last, 31);
+            if (lane == 0 && pf_prev != 0xffffffffu && k0 > pf_prev && k1 >= k0 && first + AXG_CHUNK <= n_in) {
+                const unsigned long long lo = (unsigned long long)k0 + (k0 - pf_prev) + pf_reach;
+                const unsigned long long span = min((unsigned long long)(k1 - k0) + 8ull, 4096ull);
+                if (lo + span < p.cells)
+                    axg_prefetch_l2(p.cnt + (lo & ~3ull), (uint32_t)(((span + 7ull) & ~3ull) * 4ull));
+            }
+            pf_prev = k0;
+        }
+#endif
         // O1 + P1b for the four rows first, as straight-line code (the compiler interleaves the four Philox chains);
         // the divergent part -- ranks and stores -- comes after
         uint32_t alive = 0u;
 #pragma unroll
         for (int i = 0; i < DIFF_ITEMS; ++i) {
             float z0, z1, z2;
+#ifdef AXG_PROBE_NOMATH
+            z0 = __uint_as_float((id[i] & 0x7fffffu) | 0x3f800000u) - 1.5f; z1 = -z0; z2 = z0 * 0.5f;
+#else
             axg_normals3(id[i], t, 0u, rk, z0, z1, z2);
+#endif
             x[i] = fmaf(p.sigma, z0, x[i]);
             y[i] = fmaf(p.sigma, z1, y[i]);
             z[i] = fmaf(p.sigma, z2, z[i]);
             const bool in = x[i] >= 0.0f && x[i] < p.fnx && y[i] >= 0.0f && y[i] < p.fny && z[i] >= 0.0f && z[i] < p.fnz;
-            alive |= ((first + i * 32) < n_in && in) ? (1u << i) : 0u;
+            alive |= ((first + i * 32) < n_in && in) ? (1u << i) : 0u;  // rows past n_in hold padding: never alive
         }
+#if AXG_P1_STAGES > 0
+        // every lane has its rows in registers (the arithmetic above consumed them): the stage is free for the chunk
+        // AXG_P1_STAGES trips ahead
+        __syncwarp();
+        if (lane == 0 && chunk + AXG_P1_STAGES * warps_total < n_chunks) request(chunk + AXG_P1_STAGES * warps_total, st);
+        if (++st == AXG_P1_STAGES) { st = 0; parity ^= 1u; }
+#endif
+#if AXG_P1_DEFER
+        // the {key, arrival rank} words of the PREVIOUS chunk: its counting atomics were issued before the arithmetic
+        // above, so their return values have long arrived -- no warp ever waits for an atomic round trip
+        if (have_pend) {
+#pragma unroll
+            for (int i = 0; i < DIFF_ITEMS; ++i)
+                if ((palive >> i) & 1u) p.kw[pdst[i]] = make_uint2(pkey[i], parr[i] | (((psp >> (8 * i)) & 3u) << 30));
+        }
+#endif
         uint32_t out = chunk * AXG_CHUNK;
-        uint32_t dst[DIFF_ITEMS], arr[DIFF_ITEMS];
+        uint32_t dst[DIFF_ITEMS], arr[DIFF_ITEMS], key[DIFF_ITEMS];
 #pragma unroll
         for (int i = 0; i < DIFF_ITEMS; ++i) {  // P1d + P2a
             const bool a = (alive >> i) & 1u;
             const uint32_t b = __ballot_sync(0xffffffffu, a);
             dst[i] = out + __popc(b & lt);
+            key[i] = 0u;
+            arr[i] = 0u;
             if (a) {
-                const uint32_t key = axg_cell_key(p, x[i], y[i], z[i]);
-                arr[i] = atomicAdd(p.cnt + key, 1u);  // old count = arrival rank inside the cell (see tally)
+                key[i] = axg_cell_key(p, x[i], y[i], z[i]);
+#if defined(AXG_PROBE_NOATOM)
+                arr[i] = 0u;
+#elif defined(AXG_PROBE_RED)
+                atomicAdd(p.cnt + key[i], 1u); arr[i] = 0u;
+#else
+                arr[i] = atomicAdd(p.cnt + key[i], 1u);  // old count = arrival rank inside the cell (see tally)
+#endif
+#ifndef AXG_PROBE_NOSTORE
                 p.Brec[dst[i]] = make_float4(x[i], y[i], z[i], __uint_as_float(id[i]));
-                p.key_pre[dst[i]] = key;
+#endif
             }
             out += __popc(b);
         }
+#if AXG_P1_DEFER
+        have_pend = true;
+        palive = alive;
+        psp = sp[0] | (sp[1] << 8) | (sp[2] << 16) | (sp[3] << 24);
+#pragma unroll
+        for (int i = 0; i < DIFF_ITEMS; ++i) { pdst[i] = dst[i]; parr[i] = arr[i]; pkey[i] = key[i]; }
+#else
 #pragma unroll
         for (int i = 0; i < DIFF_ITEMS; ++i)  // the four atomics have been in flight together: one wait, not four
-            if ((alive >> i) & 1u) p.arr_pre[dst[i]] = arr[i] | (sp[i] << 30);  // species in the top two bits; (storing
-                                                                                // them a trip later gains nothing: measured)
+#ifndef AXG_PROBE_NOSTORE
+            if ((alive >> i) & 1u) p.kw[dst[i]] = make_uint2(key[i], arr[i] | (sp[i] << 30));  // species: top two bits
+#else
+            if (((alive >> i) & 1u) && key[i] + arr[i] + sp[i] == 0xfffffff7u) p.kw[dst[i]] = make_uint2(key[i], arr[i]);
+#endif
+#endif
         if (lane == 0) {
             const uint32_t c = out - chunk * AXG_CHUNK;
             p.chunk_cnt[chunk] = c;
             mine += c;
         }
     }
+#if AXG_P1_DEFER
+    if (have_pend) {
+#pragma unroll
+        for (int i = 0; i < DIFF_ITEMS; ++i)
+            if ((palive >> i) & 1u) p.kw[pdst[i]] = make_uint2(pkey[i], parr[i] | (((psp >> (8 * i)) & 3u) << 30));
+    }
+#endif
     if (lane == 0 && mine) atomicAdd(&s_surv, mine);
     __syncthreads();
     if (tid == 0 && s_surv) atomicAdd(&dev->n_surv, s_surv);
     if (axg_last_block(dev)) {  // every block's survivors, keys and counts are visible here
         if (tid == 0) dev->done = 0u;
         __threadfence();
-        emit_and_close(p, 1, s_hist);
+        emit_and_close(p, 1, reinterpret_cast<uint32_t(*)[AXG_RADIX]>(s_raw));
     }
 }
 
@@ -376,11 +518,17 @@ __global__ void __launch_bounds__(256) k_rekey(const AxgParams p) {
     __syncthreads();
     for (uint32_t g = blockIdx.x * blockDim.x + threadIdx.x; g < n; g += gridDim.x * blockDim.x) {
         const float x = p.A.x[g], y = p.A.y[g], z = p.A.z[g];
-        const uint32_t key = axg_cell_key(p, x, y, z);
+        // axg_load_particles does not validate positions: a row outside the domain has no cell.  It is flagged (the
+        // call reports AXG_EINVAL) and binned into cell 0 so that nothing is written out of bounds.
+        const bool in = x >= 0.0f && x < p.fnx && y >= 0.0f && y < p.fny && z >= 0.0f && z < p.fnz;
+        if (!in) atomicOr(&dev->err, 4u);
+        const uint32_t key = in ? axg_cell_key(p, x, y, z) : 0u;
         p.Brec[g] = make_float4(x, y, z, __uint_as_float(p.A.id[g]));
         const uint32_t sp = p.A.species[g];
-        if (p.bin_mode != AXG_BIN_COUNT_D) p.Bsp[g] = (uint8_t)sp;
-        p.key_pre[g] = key;
+        if (p.bin_mode != AXG_BIN_COUNT_D) {
+            p.Bsp[g] = (uint8_t)sp;
+            p.key_pre[g] = key;
+        }
         if (p.bin_mode == AXG_BIN_COUNT_D && (g % AXG_CHUNK) == 0u) p.chunk_cnt[g / AXG_CHUNK] = min(AXG_CHUNK, n - g);
         tally(p, s_hist, key, g, sp);
     }
@@ -402,8 +550,21 @@ __global__ void __launch_bounds__(EMIT_THREADS) k_emit(const AxgParams p, int do
 int axg_diffuse_tile() { return DIFF_TILE; }
 
 void axg_launch_diffuse(const AxgParams& p, int grid, cudaStream_t s) {
-    if (p.bin_mode == AXG_BIN_COUNT_D) k_diffuse_chunked<<<148 * AXG_CHUNKED_BLOCKS, DIFF_THREADS, 0, s>>>(p);
-    else k_diffuse<<<grid, DIFF_THREADS, 0, s>>>(p);
+    if (p.bin_mode == AXG_BIN_COUNT_D) {
+        static bool attr_set = false;  // dynamic shared memory above 48 KB needs the opt-in once per process
+        if (!attr_set) {
+            cudaFuncSetAttribute(k_diffuse_chunked, cudaFuncAttributeMaxDynamicSharedMemorySize, P1_SMEM);
+            attr_set = true;
+        }
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(148 * AXG_CHUNKED_BLOCKS);
+        cfg.blockDim = dim3(DIFF_THREADS);
+        cfg.dynamicSmemBytes = P1_SMEM;
+        cfg.stream = s;
+        cudaLaunchKernelEx(&cfg, k_diffuse_chunked, p);
+    } else {
+        k_diffuse<<<grid, DIFF_THREADS, 0, s>>>(p);
+    }
 }
 void axg_launch_rekey(const AxgParams& p, int grid, cudaStream_t s) { k_rekey<<<grid, 256, 0, s>>>(p); }
 void axg_launch_emit(const AxgParams& p, int do_emit, cudaStream_t s) { k_emit<<<1, EMIT_THREADS, 0, s>>>(p, do_emit); }

@@ -8,13 +8,13 @@ bit-identical on every rank.  No particle ever moves between ranks.
 
 Host logic only (no arithmetic of the method): the loop drives any object with the boundary's call names -- the
 CUDA binding (NCCL all-reduce on the device buffer, no host synchronisation inside the loop) or, in the world_size-2
-`gloo` tests, the CPU oracle binding.
+`gloo` tests, any other object with the same calls and an exchange function of the test's own.
 """
 from __future__ import annotations
 
 import numpy as np
 
-PHASE_DIFFUSE, PHASE_BIN, PHASE_SENSE, PHASE_ADVANCE, PHASE_COMMIT = 1, 2, 4, 8, 16
+PHASE_DIFFUSE, PHASE_BIN, PHASE_SENSE, PHASE_ADVANCE, PHASE_COMMIT, PHASE_CONNECT = 1, 2, 4, 8, 16, 32
 
 
 class _DevBuf:
@@ -38,39 +38,87 @@ def nccl_exchange(sim):
     return run
 
 
-def host_exchange(sim):
-    """The same exchange for a binding whose sums live on the host (oracle): read -> all-reduce (gloo) -> load."""
-    import torch
-    import torch.distributed as dist
-
-    def run():
-        c = torch.from_numpy(sim.read_state("CONE_COUNTS").astype(np.int64))
-        m = torch.from_numpy(sim.read_state("CONE_MOMENT").astype(np.int64))
-        if c.numel() == 0:
-            return
-        # frozen cones keep stale sums on every rank; they are not read by P4, only kept consistent here
-        dist.all_reduce(c, op=dist.ReduceOp.SUM)
-        dist.all_reduce(m, op=dist.ReduceOp.SUM)
-        sim.load_sense(c.numpy(), m.numpy())
-    return run
-
-
 class ShardedStepper:
-    """`step(n)` of a simulation sharded over `world` ranks.  `exchange` is nccl_exchange or host_exchange."""
+    """`step(n)` of a simulation sharded over `world` ranks.  `exchange(sim)` returns the callable that all-reduces the
+    per-cone sums between P3 and P4 (nccl_exchange here; the CPU tests pass their own).
 
-    def __init__(self, sim, rank, world, exchange):
+    With the CUDA binding (an object that has `enqueue_phase_on`) the loop is the one `axg_step` runs on one GPU, with
+    the all-reduce in it: P3, the all-reduce and P4 / P5 of step t go to a side stream BESIDE P1 of step t+1 on the main
+    stream (they share no data), joined before P2 of step t+1; for n >= 4 one such unit is captured once as a CUDA graph
+    (NCCL collectives are capturable) and replayed, re-captured when `params_fingerprint` says a launch would be stale.
+    Bindings without streams (the oracle in the gloo tests) run the plain sequence."""
+
+    GRAPH_MIN_STEPS = 4
+
+    def __init__(self, sim, rank, world, exchange, overlap=None, graph=True):
         self.sim, self.rank, self.world = sim, int(rank), int(world)
         sim.set_shard(self.rank, self.world)
         self._exchange = exchange(sim) if self.world > 1 else (lambda: None)
+        self._overlap = hasattr(sim, "enqueue_phase_on") if overlap is None else bool(overlap)
+        self._use_graph = bool(graph)
+        self._side = None
+        self._graph = None
+        self._graph_fp = None
+        self._graph_stream = None
 
-    def step(self, n=1):
+    # ---- plain sequence (any binding) ----------------------------------------------------------------------------
+    def _step_plain(self, n):
         sim = self.sim
-        sim.check_capacity(n)
         for _ in range(n):
             sim.enqueue_phase(PHASE_DIFFUSE | PHASE_BIN | PHASE_SENSE)
             self._exchange()
-            sim.enqueue_phase(PHASE_ADVANCE | PHASE_COMMIT)
-        sim.sync()
+            sim.enqueue_phase(PHASE_ADVANCE | PHASE_CONNECT | PHASE_COMMIT)
+
+    # ---- overlapped sequence (CUDA binding) ---------------------------------------------------------------------------
+    def _cones(self, stream, torch):
+        sim = self.sim
+        sim.enqueue_phase_on(PHASE_SENSE, stream.cuda_stream)
+        with torch.cuda.stream(stream):
+            self._exchange()
+        sim.enqueue_phase_on(PHASE_ADVANCE | PHASE_CONNECT | PHASE_COMMIT, stream.cuda_stream, overlapped=True)
+
+    def _unit(self, main, prev_cones, torch):
+        """[cones of the previous step on the side stream || P1 of this step] -> P2 of this step"""
+        sim = self.sim
+        if prev_cones:
+            self._side.wait_stream(main)
+            self._cones(self._side, torch)
+        sim.enqueue_phase_on(PHASE_DIFFUSE, main.cuda_stream)
+        if prev_cones:
+            main.wait_stream(self._side)
+        sim.enqueue_phase_on(PHASE_BIN, main.cuda_stream)
+
+    def _step_overlapped(self, n):
+        import torch
+        main = torch.cuda.current_stream()
+        if self._side is None:
+            self._side = torch.cuda.Stream()
+        self._unit(main, False, torch)
+        rest = n - 1
+        if rest > 0 and self._use_graph and n >= self.GRAPH_MIN_STEPS:
+            fp = self.sim.params_fingerprint()
+            if self._graph is None or self._graph_fp != fp:
+                g = torch.cuda.CUDAGraph()
+                torch.cuda.synchronize()
+                with torch.cuda.graph(g, capture_error_mode="thread_local"):
+                    self._unit(torch.cuda.current_stream(), True, torch)
+                self._graph, self._graph_fp = g, fp
+            for _ in range(rest):
+                self._graph.replay()
+        else:
+            for _ in range(rest):
+                self._unit(main, True, torch)
+        self._cones(main, torch)      # P3..P5 of the last step
+
+    def step(self, n=1):
+        if n <= 0:
+            return
+        self.sim.check_capacity(n)
+        if self._overlap:
+            self._step_overlapped(n)
+        else:
+            self._step_plain(n)
+        self.sim.sync()
 
 
 def owned_sources(n_sources, rank, world):

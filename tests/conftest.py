@@ -32,3 +32,15 @@ def pytest_collection_modifyitems(config, items):
 @pytest.fixture(scope="session")
 def golden_dir():
     return os.path.join(ROOT, "tests", "golden")
+
+
+def pytest_terminal_summary(terminalreporter):
+    """What the parity comparisons actually saw (survivor flips near walls, fraction of the tolerance used)."""
+    try:
+        import parity_util as pu
+    except Exception:
+        return
+    if pu.REPORT:
+        terminalreporter.write_line("parity report (tests/parity_util.py):")
+        for line in pu.REPORT:
+            terminalreporter.write_line("  " + line)

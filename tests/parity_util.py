@@ -7,6 +7,12 @@ from paper_1405_3331_b200 import workloads as W
 RTOL, ATOL = 1e-5, 1e-6   # BASELINE.json north_star: single-step fp32 positions, gradients, headings
 BINNING = None            # axg.BIN_RADIX / axg.BIN_COUNT: set by the parametrised fixture of the GPU tests
 KEY_ORDER = 0             # 1: both sides use the bricked cell order (include/axg.h axg_set_key_order)
+# Reading A-19: a GPU position within rounding of a wall may be absorbed on one side only.  Expected rate
+# with the accurate Box-Muller of both sides: ~5e-7 per particle-step; accepted: 4x that, and
+# never fewer than 4 (small cases).  Every comparison appends what it saw to REPORT (printed by conftest.py at the end
+# of the run): flips and the largest fraction of the position tolerance that was used.
+FLIP_RATE_MAX = 2e-6
+REPORT = []
 
 
 def new_axg(axg_mod, *args):
@@ -41,7 +47,7 @@ def close(a, b):
     return np.abs(a.astype(np.float64) - b.astype(np.float64)) <= ATOL + RTOL * np.abs(b.astype(np.float64))
 
 
-def near_wall(x, y, z, grid, tol_scale=4.0):
+def near_wall(x, y, z, grid, tol_scale=1.0):
     """True where a coordinate is within the comparison tolerance of a domain wall (reading A-19)."""
     out = np.zeros(x.shape, dtype=bool)
     for v, n in ((x, grid[0]), (y, grid[1]), (z, grid[2])):
@@ -51,7 +57,7 @@ def near_wall(x, y, z, grid, tol_scale=4.0):
     return out
 
 
-def compare_presort(gp, op, grid, n_newborn):
+def compare_presort(gp, op, grid, n_newborn, label=None):
     """P1 parity (reading A-19): ids and their order equal except for particles that one side absorbed and the other
     kept within tolerance of a wall; positions of the common ids within tolerance.  Returns the number of flips."""
     gid, oid = gp["ID"], op["ID"]
@@ -62,22 +68,27 @@ def compare_presort(gp, op, grid, n_newborn):
         only_g = np.setdiff1d(gid, oid)
         only_o = np.setdiff1d(oid, gid)
         flips = len(only_g) + len(only_o)
-        assert flips <= max(4, int(2e-5 * len(oid))), "too many survivor mismatches: %d" % flips
+        assert flips <= max(4, int(FLIP_RATE_MAX * len(oid))), "too many survivor mismatches: %d of %d" % (flips, len(oid))
         mg = np.isin(gid, only_g)
         mo = np.isin(oid, only_o)
         assert near_wall(gp["X"][mg], gp["Y"][mg], gp["Z"][mg], grid).all()
         assert near_wall(op["X"][mo], op["Y"][mo], op["Z"][mo], grid).all()
         common_g, common_o = ~mg, ~mo
         assert np.array_equal(gid[common_g], oid[common_o]), "order of the common survivors differs"
+    used = 0.0
     for k in ("X", "Y", "Z"):
-        bad = ~close(gp[k][common_g], op[k][common_o])
-        assert not bad.any(), "%s: %d positions out of tolerance, worst %g" % (
-            k, bad.sum(), np.abs(gp[k][common_g] - op[k][common_o]).max())
+        a, b = gp[k][common_g].astype(np.float64), op[k][common_o].astype(np.float64)
+        frac = np.abs(a - b) / (ATOL + RTOL * np.abs(b))
+        bad = frac > 1.0
+        assert not bad.any(), "%s: %d positions out of tolerance, worst %g" % (k, bad.sum(), np.abs(a - b).max())
+        used = max(used, float(frac.max()) if frac.size else 0.0)
     assert np.array_equal(gp["SPECIES"][common_g], op["SPECIES"][common_o])
     if n_newborn and flips == 0:
         # newborns sit exactly at their source on both sides: bit-equal
         for k in ("X", "Y", "Z"):
             assert np.array_equal(gp[k][-n_newborn:], op[k][-n_newborn:])
+    REPORT.append("P1 %-28s n=%-10d flips=%-3d (accepted %d)  worst |dx| = %.3f of the tolerance" % (
+        label or "", len(oid), flips, max(4, int(FLIP_RATE_MAX * len(oid))), used))
     return flips
 
 

@@ -62,6 +62,8 @@ def test_one_call_equals_many_calls(axg, binning):
     mode = axg.BIN_COUNT if binning == "count" else axg.BIN_RADIX
     _same(_run(axg, mode, [STEPS]), _run(axg, mode, [1] * STEPS))
     _same(_run(axg, mode, [STEPS]), _run(axg, mode, [7, 1, 22]))
+    # n = 2, 3: the overlapped path without the CUDA graph (enqueue_phases with P3..P5 on the side stream)
+    _same(_run(axg, mode, [STEPS]), _run(axg, mode, [2, 3, 2, 3, 3, 2, 15]))
 
 
 def test_count_binning_equals_radix_binning(axg):
@@ -170,17 +172,32 @@ def test_sharded_stepper_with_a_real_nccl_all_reduce(axg):
             W.apply(g, w)
             return g
 
-        ref, g = make(), make()
+        ref, g, h = make(), make(), make()
         ref.step(25)
         st = S.ShardedStepper(g, 0, 1, S.nccl_exchange)
         st._exchange = S.nccl_exchange(g)   # with one rank the stepper would skip the exchange: force it
-        st.step(25)
+        assert st._overlap                  # the CUDA binding takes the overlapped, graph-captured loop
+        st.step(25)                         # first unit eager, 24 replays of the captured unit, last cones eager
         torch.cuda.synchronize()
         for f in FIELDS:
             a, b = ref.read_state(f), g.read_state(f)
             assert np.array_equal(a.view(np.uint8), b.view(np.uint8)), f
+        # every call pattern of the loop: plain (n = 1), overlapped without a graph (n = 2, 3), graph (n >= 4), and the
+        # same stepper again after the context's parameters changed (the captured unit must be re-captured)
+        st2 = S.ShardedStepper(h, 0, 1, S.nccl_exchange)
+        st2._exchange = S.nccl_exchange(h)
+        for n in (1, 2, 3, 5, 6):
+            st2.step(n)
+        h.set_capacity(w.max_particles + 4096, w.max_segments)
+        st2.step(8)
+        torch.cuda.synchronize()
+        assert h.counters()["step"] == 25
+        for f in FIELDS:
+            a, b = ref.read_state(f), h.read_state(f)
+            assert np.array_equal(a.view(np.uint8), b.view(np.uint8)), f
         ref.close()
         g.close()
+        h.close()
     finally:
         if own_group:
             dist.destroy_process_group()

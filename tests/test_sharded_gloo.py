@@ -23,6 +23,21 @@ if ROOT not in sys.path:
 STEPS = 6
 
 
+def host_exchange(sim):
+    """The exchange step of the sharded loop for a binding whose sums live on the host (the oracle): read -> all-reduce
+    (gloo) -> load.  Test harness only: the product's exchange is sharded.nccl_exchange on the device buffer."""
+    def run():
+        c = torch.from_numpy(sim.read_state("CONE_COUNTS").astype(np.int64))
+        m = torch.from_numpy(sim.read_state("CONE_MOMENT").astype(np.int64))
+        if c.numel() == 0:
+            return
+        # frozen cones keep stale sums on every rank; they are not read by P4, only kept consistent here
+        dist.all_reduce(c, op=dist.ReduceOp.SUM)
+        dist.all_reduce(m, op=dist.ReduceOp.SUM)
+        sim.load_sense(c.numpy(), m.numpy())
+    return run
+
+
 def _workload():
     from paper_1405_3331_b200 import workloads as W
     w = W.small(seed=21, grid=(20, 18, 14), n_cones=40, n_sources=5, rate=60)
@@ -53,7 +68,7 @@ def _worker(rank, world, port, q, sensing):
         from paper_1405_3331_b200 import sharded
         w = _workload()
         o = _oracle(w, sensing)
-        stepper = sharded.ShardedStepper(o, rank, world, sharded.host_exchange)
+        stepper = sharded.ShardedStepper(o, rank, world, host_exchange)
         stepper.step(STEPS)
         st = _state(o)
         q.put((rank, {k: (v if isinstance(v, dict) else v.tolist()) for k, v in st.items()}))
