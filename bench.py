@@ -66,10 +66,11 @@ def measured_peak():
 # algorithmic bytes: what the method must move per particle and per step
 # ---------------------------------------------------------------------------------------------------------------
 def key_passes(cells):
+    """digit passes of the radix sort: 8-bit digits, 9-bit where that saves a pass (axg_api.cu digit_bits_for)"""
     bits = 1
     while bits < 32 and (1 << bits) < cells:
         bits += 1
-    return (bits + 7) // 8
+    return min((bits + 7) // 8, (bits + 8) // 9)
 
 
 def bytes_model(w, n_live, n_active_cones, n_stencil, count_mode):

@@ -169,10 +169,15 @@ uint64_t owned_rate(const axg_ctx* c) {
     return e;
 }
 
-int key_passes(size_t cells) {
+int key_bits(size_t cells) {
     int bits = 1;
     while (bits < 32 && ((size_t)1 << bits) < cells) ++bits;
-    return (bits + 7) / 8;
+    return bits;
+}
+// 9-bit digits where they save a pass (27-bit keys: C4), 8-bit otherwise (one ballot less per key)
+int digit_bits_for(size_t cells) {
+    const int b = key_bits(cells);
+    return (b + 8) / 9 < (b + 7) / 8 ? 9 : 8;
 }
 
 // ---- allocation ------------------------------------------------------------------------------------------
@@ -230,7 +235,8 @@ int alloc_fixed(axg_ctx* c) {
     P.sigma = (float)std::sqrt(2.0 * (double)c->D);  // O0
     P.seed_lo = (uint32_t)(c->seed & 0xffffffffull);
     P.seed_hi = (uint32_t)(c->seed >> 32);
-    P.n_pass = key_passes(c->cells());
+    P.digit_bits = digit_bits_for(c->cells());
+    P.n_pass = (key_bits(c->cells()) + P.digit_bits - 1) / P.digit_bits;
     P.final_buf = (P.n_pass - 1) & 1;
     P.src = (const AxgSourceDev*)c->d_src;
     P.src_id_prefix = (const uint32_t*)c->d_src_id_prefix;
@@ -259,7 +265,7 @@ int alloc_particles(axg_ctx* c, uint64_t cap, AxgParams& P, std::vector<void*>& 
     const size_t sizes[] = {n * 4, n * 4, n * 4, n, n * 4,  // A (SoA)
                             n * 16, n,                      // Brec, Bsp
                             n * 8, n * 4, n * 4, n * 4, n * 4,  // key_pre (radix) = kw (count: key + arrival rank), skey[2], sidx[2]
-                            diff_tiles * 8, sort_tiles * AXG_RADIX * 8,
+                            diff_tiles * 8, sort_tiles * ((size_t)1 << P.digit_bits) * 8,
                             (n / AXG_CHUNK + 4) * 4, (n / AXG_CHUNK + 4) * 4,   // chunk_cnt, chunk_base
                             (n / 33 + 64) * 4, AXG_MAX_SOURCES * 4};            // big_list, src_arr
     constexpr int NB = 18;

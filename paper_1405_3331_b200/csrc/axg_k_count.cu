@@ -222,9 +222,6 @@ constexpr int PLACE_THREADS = 256;
 // occupancy) but as a whole, by one block (settle_big_cell below).  k_place lists them: the row whose arrival rank is
 // exactly SETTLE_INLINE exists once in every cell with more than SETTLE_INLINE members.
 constexpr uint32_t SETTLE_INLINE = 32u;
-#ifndef AXG_PLACE_PREFETCH
-#define AXG_PLACE_PREFETCH 1
-#endif
 
 __global__ void __launch_bounds__(PLACE_THREADS) k_place(const AxgParams p) {
     // B is in the chunked layout of k_diffuse_chunked: every physical row below n_pp is visited, the holes at the end
@@ -235,31 +232,7 @@ __global__ void __launch_bounds__(PLACE_THREADS) k_place(const AxgParams p) {
     // one particle per thread: the kernel is bound by L2 transactions (one random 4-byte read of the cell start + one
     // scattered 4-byte store each) and wants many warps in flight.  No atomic: the counting atomic of P1 already
     // returned every row's arrival rank inside its cell (kw.y), in the arbitrary order of the atomics.
-#if AXG_PLACE_PREFETCH
-    // the first touch of a sector of cell_lo is a random read at DRAM latency: sweep cell_lo into the L2 one grid sweep
-    // (+ the reach of a particle's move) ahead, as k_diffuse_chunked does for cnt
-    uint32_t pf_prev = 0xffffffffu;
-    const uint32_t pf_reach = (uint32_t)min((float)p.cells, (6.0f * p.sigma + 1.5f) * (p.key_order == 0 ? (float)p.nx * (float)p.ny
-                                                                                                : 4096.0f));
-#endif
     for (uint32_t o = blockIdx.x * PLACE_THREADS + threadIdx.x; o < n_pp; o += gridDim.x * PLACE_THREADS) {
-#if AXG_PLACE_PREFETCH
-        {   // warp-uniform: every lane of the warp is inside the loop (n_pp is padded by the grid-stride test below)
-            const uint32_t act = __activemask();
-            const uint32_t kk = __ldg(&p.kw[o].x);
-            const int leader = __ffs(act) - 1, last = 31 - __clz(act);
-            const uint32_t k0 = __shfl_sync(act, kk, leader), k1 = __shfl_sync(act, kk, last);
-            if ((threadIdx.x & 31) == leader) {
-                // keys of a chunk's survivors are those of neighbouring input rows +- the move: take the span generously
-                if (pf_prev != 0xffffffffu && k0 > pf_prev) {
-                    const unsigned long long lo = (unsigned long long)k0 + (k0 - pf_prev) + pf_reach;
-                    if (lo + 64ull < p.cells) axg_prefetch_l2(cell_lo + (lo & ~3ull), 256u);
-                }
-                pf_prev = k0;
-            }
-            (void)k1;
-        }
-#endif
         if (o < n_phys && (o % AXG_CHUNK) >= __ldg(p.chunk_cnt + o / AXG_CHUNK)) continue;  // a hole
         const uint2 w = __ldg(p.kw + o);  // key, arrival rank | species << 30: one 8-byte load
         const uint32_t arr = w.y & AXG_IDX_MASK;
@@ -278,7 +251,7 @@ constexpr int SETTLE_ITEMS = 1;  // warp-striped (item i of lane l is slot base 
 #endif
 constexpr uint32_t SETTLE_SORT_MAX = AXG_SETTLE_SORT_MAX;
 #ifndef AXG_SETTLE_PREFETCH
-#define AXG_SETTLE_PREFETCH 5   // look-ahead of the record prefetch in half grid sweeps (0 = off)
+#define AXG_SETTLE_PREFETCH 3   // look-ahead of the record prefetch in half grid sweeps (0 = off)
 #endif  // members of a cell that one block sorts in shared memory
 
 template <bool WITH_KP>

@@ -26,7 +26,7 @@ __device__ __forceinline__ void tally(const AxgParams& p, uint32_t (*s_hist)[AXG
     } else {
 #pragma unroll
         for (int q = 0; q < AXG_MAX_PASSES; ++q)
-            if (q < p.n_pass) atomicAdd(&s_hist[q][(key >> (8 * q)) & 0xffu], 1u);
+            if (q < p.n_pass) atomicAdd(&s_hist[q][(key >> (p.digit_bits * q)) & ((1u << p.digit_bits) - 1u)], 1u);
     }
 }
 
@@ -86,28 +86,36 @@ __device__ void emit_and_close(const AxgParams& p, int do_emit, uint32_t (*s_his
         }
     }
     if (p.bin_mode != AXG_BIN_COUNT_D) {
-        // total histogram -> exclusive scan per pass; needs >= 256 threads (one digit each)
+        // total histogram -> exclusive scan per pass: the block's 256 threads take the digits 256 at a time
+        const int n_digits = 1 << p.digit_bits;
         for (int q = 0; q < p.n_pass; ++q) {
-            const int d = tid, lane = tid & 31, wq = tid >> 5;
-            uint32_t c = 0u, inc = 0u;
-            if (d < AXG_RADIX) {
-                c = dev->hist[q][d] + s_hist[q][d];
-                inc = c;
+            uint32_t carry = 0u;
+            for (int d0 = 0; d0 < n_digits; d0 += 256) {
+                const int d = d0 + tid, lane = tid & 31, wq = tid >> 5;
+                uint32_t c = 0u, inc = 0u;
+                if (tid < 256) {
+                    c = dev->hist[q][d] + s_hist[q][d];
+                    inc = c;
 #pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o);
-                    if (lane >= o) inc += v;
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o);
+                        if (lane >= o) inc += v;
+                    }
+                    if (lane == 31) s_scan[wq] = inc;
                 }
-                if (lane == 31) s_scan[wq] = inc;
+                __syncthreads();
+                uint32_t off = 0u, total = 0u;
+                for (int w = 0; w < 8; ++w) {
+                    off += w < wq ? s_scan[w] : 0u;
+                    total += s_scan[w];
+                }
+                if (tid < 256) {
+                    dev->base[q][d] = carry + off + inc - c;
+                    dev->hist[q][d] = 0u;
+                }
+                carry += total;
+                __syncthreads();
             }
-            __syncthreads();
-            if (d < AXG_RADIX) {
-                uint32_t off = 0u;
-                for (int w = 0; w < wq; ++w) off += s_scan[w];
-                dev->base[q][d] = off + inc - c;
-                dev->hist[q][d] = 0u;
-            }
-            __syncthreads();
         }
     }
     if (tid == 0 && !do_emit) {  // harness path after k_rekey: B is dense, which is a valid chunked layout too
@@ -286,21 +294,19 @@ __global__ void __launch_bounds__(DIFF_THREADS, 4) k_diffuse(const AxgParams p) 
 #ifndef AXG_CHUNKED_BLOCKS
 #define AXG_CHUNKED_BLOCKS 4
 #endif
-#ifndef AXG_P1_DEFER
-#define AXG_P1_DEFER 1    // store a chunk's {key, arrival rank} words one trip later (the atomics' round trip is hidden)
-#endif
-#ifndef AXG_P1_PREFETCH
-#define AXG_P1_PREFETCH 1  // sweep the count array into the L2 ahead of the counting atomics (see the kernel)
+#ifndef AXG_P1_DYNAMIC
+#define AXG_P1_DYNAMIC 1
 #endif
 #ifndef AXG_P1_STAGES
-#define AXG_P1_STAGES 2   // chunks in flight per warp (bulk-async staging); 0 = per-lane loads held in registers
+#define AXG_P1_STAGES 0   // chunks in flight per warp (bulk-async staging); 0 = per-lane loads held in registers
 #endif
 // One stage = the five column runs of one chunk: x, y, z, id (512 B each) and species (128 B).  A chunk column is one
 // 16-byte-aligned run of global memory, so each is ONE 1-D bulk copy (cp.async.bulk -> SASS UBLKCP) whose completion
 // is counted on the stage's mbarrier: the bytes in flight no longer sit in registers behind the scoreboard, and a warp
 // only ever waits for data that was requested two chunks ago.
 constexpr int P1_STAGE_BYTES = 4 * 512 + 128;
-constexpr int P1_SMEM = DIFF_WARPS * (AXG_P1_STAGES > 0 ? AXG_P1_STAGES : 1) * P1_STAGE_BYTES;
+constexpr int P1_SMEM = AXG_P1_STAGES > 0 ? DIFF_WARPS * AXG_P1_STAGES * P1_STAGE_BYTES
+                                          : (int)(AXG_MAX_PASSES * AXG_RADIX * sizeof(uint32_t));  // scratch of emit_and_close
 static_assert(P1_SMEM >= (int)(AXG_MAX_PASSES * AXG_RADIX * sizeof(uint32_t)), "emit_and_close reuses the staging area");
 
 __global__ void __launch_bounds__(DIFF_THREADS, AXG_CHUNKED_BLOCKS) k_diffuse_chunked(const AxgParams p) {
@@ -345,20 +351,19 @@ __global__ void __launch_bounds__(DIFF_THREADS, AXG_CHUNKED_BLOCKS) k_diffuse_ch
     uint32_t parity = 0u;
 #endif
     __syncthreads();  // s_surv
-#if AXG_P1_PREFETCH
-    uint32_t pf_prev = 0xffffffffu;
-    // how far beyond its own cell a particle's counting atomic can land: 6 sigma in z (planes of nx ny cells; linear key)
-    const uint32_t pf_reach = (uint32_t)min((float)p.cells, (6.0f * p.sigma + 1.5f) * (p.key_order == 0 ? (float)p.nx * (float)p.ny
-                                                                                                : 4096.0f));
-#endif
-#if AXG_P1_DEFER
-    bool have_pend = false;
-    uint32_t palive = 0u, psp = 0u, pdst[DIFF_ITEMS], parr[DIFF_ITEMS], pkey[DIFF_ITEMS];
-#pragma unroll
-    for (int i = 0; i < DIFF_ITEMS; ++i) { pdst[i] = 0u; parr[i] = 0u; pkey[i] = 0u; }
-#endif
 
+#if AXG_P1_DYNAMIC && AXG_P1_STAGES == 0
+    // Chunks are handed out by a device ticket, one per warp trip, drawn one trip ahead (its latency hides behind the
+    // arithmetic): SMs differ in speed (distance to the L2 slices, the other die), and with a fixed share per warp the
+    // fast ones idle at the end -- 11 % of the warp slots in the profile of the static loop.
+    uint32_t next_chunk = 0u;
+    if (lane == 0) next_chunk = atomicAdd(&dev->ticket, 1u);
+    next_chunk = __shfl_sync(0xffffffffu, next_chunk, 0);
+    for (uint32_t chunk = next_chunk; chunk < n_chunks; chunk = next_chunk) {
+        if (lane == 0) next_chunk = atomicAdd(&dev->ticket, 1u);
+#else
     for (uint32_t chunk = gw; chunk < n_chunks; chunk += warps_total) {
+#endif
         const uint32_t first = chunk * AXG_CHUNK + lane;
         float x[DIFF_ITEMS], y[DIFF_ITEMS], z[DIFF_ITEMS];
         uint32_t id[DIFF_ITEMS], sp[DIFF_ITEMS];
@@ -394,37 +399,13 @@ __global__ void __launch_bounds__(DIFF_THREADS, AXG_CHUNKED_BLOCKS) k_diffuse_ch
             }
         }
 #endif
-#if AXG_P1_PREFETCH
-        // A counting atomic on a sector of cnt that is not in the L2 waits for DRAM (one in eight: a sector holds eight
-        // cells and each cell gets about one particle).  All warps sweep the sorted input in step, so the keys that the
-        // NEXT trip of this warp will hit lie one sweep ahead of the keys of this trip, +- the few cell planes a particle
-        // moves: every warp asks for its own span of cnt, shifted by (one sweep + that reach), with one bulk L2 prefetch.
-        // The sweep length in keys is measured from the warp's own previous trip.
-        {
-            const uint32_t k_first = axg_cell_key(p, fmaxf(x[0], 0.0f), fmaxf(y[0], 0.0f), fmaxf(z[0], 0.0f));
-            const uint32_t k_last = axg_cell_key(p, fmaxf(x[DIFF_ITEMS - 1], 0.0f), fmaxf(y[DIFF_ITEMS - 1], 0.0f),
-                                                 fmaxf(z[DIFF_ITEMS - 1], 0.0f));
-            const uint32_t k0 = __shfl_sync(0xffffffffu, k_first, 0), k1 = __shfl_sync(0xffffffffu, k_last, 31);
-            if (lane == 0 && pf_prev != 0xffffffffu && k0 > pf_prev && k1 >= k0 && first + AXG_CHUNK <= n_in) {
-                const unsigned long long lo = (unsigned long long)k0 + (k0 - pf_prev) + pf_reach;
-                const unsigned long long span = min((unsigned long long)(k1 - k0) + 8ull, 4096ull);
-                if (lo + span < p.cells)
-                    axg_prefetch_l2(p.cnt + (lo & ~3ull), (uint32_t)(((span + 7ull) & ~3ull) * 4ull));
-            }
-            pf_prev = k0;
-        }
-#endif
         // O1 + P1b for the four rows first, as straight-line code (the compiler interleaves the four Philox chains);
         // the divergent part -- ranks and stores -- comes after
         uint32_t alive = 0u;
 #pragma unroll
         for (int i = 0; i < DIFF_ITEMS; ++i) {
             float z0, z1, z2;
-#ifdef AXG_PROBE_NOMATH
-            z0 = __uint_as_float((id[i] & 0x7fffffu) | 0x3f800000u) - 1.5f; z1 = -z0; z2 = z0 * 0.5f;
-#else
             axg_normals3(id[i], t, 0u, rk, z0, z1, z2);
-#endif
             x[i] = fmaf(p.sigma, z0, x[i]);
             y[i] = fmaf(p.sigma, z1, y[i]);
             z[i] = fmaf(p.sigma, z2, z[i]);
@@ -438,15 +419,6 @@ __global__ void __launch_bounds__(DIFF_THREADS, AXG_CHUNKED_BLOCKS) k_diffuse_ch
         if (lane == 0 && chunk + AXG_P1_STAGES * warps_total < n_chunks) request(chunk + AXG_P1_STAGES * warps_total, st);
         if (++st == AXG_P1_STAGES) { st = 0; parity ^= 1u; }
 #endif
-#if AXG_P1_DEFER
-        // the {key, arrival rank} words of the PREVIOUS chunk: its counting atomics were issued before the arithmetic
-        // above, so their return values have long arrived -- no warp ever waits for an atomic round trip
-        if (have_pend) {
-#pragma unroll
-            for (int i = 0; i < DIFF_ITEMS; ++i)
-                if ((palive >> i) & 1u) p.kw[pdst[i]] = make_uint2(pkey[i], parr[i] | (((psp >> (8 * i)) & 3u) << 30));
-        }
-#endif
         uint32_t out = chunk * AXG_CHUNK;
         uint32_t dst[DIFF_ITEMS], arr[DIFF_ITEMS], key[DIFF_ITEMS];
 #pragma unroll
@@ -458,52 +430,31 @@ __global__ void __launch_bounds__(DIFF_THREADS, AXG_CHUNKED_BLOCKS) k_diffuse_ch
             arr[i] = 0u;
             if (a) {
                 key[i] = axg_cell_key(p, x[i], y[i], z[i]);
-#if defined(AXG_PROBE_NOATOM)
-                arr[i] = 0u;
-#elif defined(AXG_PROBE_RED)
-                atomicAdd(p.cnt + key[i], 1u); arr[i] = 0u;
-#else
                 arr[i] = atomicAdd(p.cnt + key[i], 1u);  // old count = arrival rank inside the cell (see tally)
-#endif
-#ifndef AXG_PROBE_NOSTORE
                 p.Brec[dst[i]] = make_float4(x[i], y[i], z[i], __uint_as_float(id[i]));
-#endif
             }
             out += __popc(b);
         }
-#if AXG_P1_DEFER
-        have_pend = true;
-        palive = alive;
-        psp = sp[0] | (sp[1] << 8) | (sp[2] << 16) | (sp[3] << 24);
-#pragma unroll
-        for (int i = 0; i < DIFF_ITEMS; ++i) { pdst[i] = dst[i]; parr[i] = arr[i]; pkey[i] = key[i]; }
-#else
 #pragma unroll
         for (int i = 0; i < DIFF_ITEMS; ++i)  // the four atomics have been in flight together: one wait, not four
-#ifndef AXG_PROBE_NOSTORE
             if ((alive >> i) & 1u) p.kw[dst[i]] = make_uint2(key[i], arr[i] | (sp[i] << 30));  // species: top two bits
-#else
-            if (((alive >> i) & 1u) && key[i] + arr[i] + sp[i] == 0xfffffff7u) p.kw[dst[i]] = make_uint2(key[i], arr[i]);
-#endif
-#endif
         if (lane == 0) {
             const uint32_t c = out - chunk * AXG_CHUNK;
             p.chunk_cnt[chunk] = c;
             mine += c;
         }
-    }
-#if AXG_P1_DEFER
-    if (have_pend) {
-#pragma unroll
-        for (int i = 0; i < DIFF_ITEMS; ++i)
-            if ((palive >> i) & 1u) p.kw[pdst[i]] = make_uint2(pkey[i], parr[i] | (((psp >> (8 * i)) & 3u) << 30));
-    }
+#if AXG_P1_DYNAMIC && AXG_P1_STAGES == 0
+        next_chunk = __shfl_sync(0xffffffffu, next_chunk, 0);
 #endif
+    }
     if (lane == 0 && mine) atomicAdd(&s_surv, mine);
     __syncthreads();
     if (tid == 0 && s_surv) atomicAdd(&dev->n_surv, s_surv);
     if (axg_last_block(dev)) {  // every block's survivors, keys and counts are visible here
-        if (tid == 0) dev->done = 0u;
+        if (tid == 0) {
+            dev->done = 0u;
+            dev->ticket = 0u;
+        }
         __threadfence();
         emit_and_close(p, 1, reinterpret_cast<uint32_t(*)[AXG_RADIX]>(s_raw));
     }
