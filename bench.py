@@ -301,7 +301,7 @@ def run_ours(args, w):
 
     K, Wm = args.steps, args.warmup
     e2e_steps = max(1, min(K, args.e2e_steps))
-    w.max_segments = Wm + 2 * K + e2e_steps + 8
+    w.max_segments = 2 * Wm + 4 * K + e2e_steps + 16     # warm-up + timed + per-kernel pass, twice (radix record), + e2e
     seed = w.seed
 
     bin_req = {"auto": axg.BIN_AUTO, "radix": axg.BIN_RADIX, "count": axg.BIN_COUNT}[args.binning]
@@ -373,7 +373,7 @@ def run_ours(args, w):
 
     # ---- per-kernel CUDA-event times over K more steps (same launch configuration; events between kernels) ----
     ktimes, roof = None, None
-    if world == 1:
+    if world == 1 and not args.force_sharded_loop:     # (the sharded loop enqueues phases itself: no per-kernel events)
         sim.profile_next_step(True)
         step(K)
         ktimes = sim.kernel_times()
@@ -382,7 +382,7 @@ def run_ours(args, w):
         active = sim.counters()["active"]
     # ---- the path north_star spells out (onesweep radix passes + reorder), timed on the same state, same K ---------
     radix_rec = None
-    if world == 1 and count_mode and not args.no_radix_record:
+    if world == 1 and count_mode and not args.no_radix_record and not args.force_sharded_loop:
         sim.set_binning(axg.BIN_RADIX)
         step(Wm)
         ms_r = timed(lambda: step(K))
@@ -523,7 +523,8 @@ def run_ours(args, w):
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
-            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "strong" if world > 1 else "weak",
+            "ms_per_step": ms / K, "higher_is_better": True,
+            "scaling": args.scaling if world > 1 else "weak",
             "vs_baseline": None, "dtype": "f32+u32", "data": "synthetic",
             "config": {"workload": w.name, "grid": list(w.grid), "cones": int(len(w.neurons)),
                        "sources": len(w.sources), "n_live_start": int(n_start), "n_live_end": int(n_end),
@@ -559,6 +560,8 @@ def main():
     ap.add_argument("--sensing", default="cell", choices=("cell", "particle", "weighted"),
                     help="P3 rule: north_star's per-cell sums, or the per-particle rule of the paper's section 5.3")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--scaling", default="strong", choices=("strong", "weak"),
+                    help="N > 1: shard the fixed workload (strong), or give every rank one config's worth of sources (weak)")
     ap.add_argument("--force-sharded-loop", action="store_true",
                     help="run the multi-GPU step loop (sharded.ShardedStepper) also at N = 1, to time it against axg_step")
     ap.add_argument("--no-radix-record", action="store_true",
@@ -566,6 +569,10 @@ def main():
     args = ap.parse_args()
     from paper_1405_3331_b200 import workloads as W
     w = W.BY_NAME[args.workload]()
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.scaling == "weak" and world > 1:
+        # per-rank work fixed: `world` times the sources; max_particles is a PER-RANK capacity, so it stays
+        w = W.weak_scaled(w, world)
     if args.impl == "reference":
         if int(os.environ.get("RANK", "0")) == 0:
             run_reference(args, w)

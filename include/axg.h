@@ -173,9 +173,9 @@ int axg_load_particles(axg_ctx* ctx, const float* x, const float* y, const float
 int axg_load_cones(axg_ctx* ctx, const float* pos, const float* heading, const uint8_t* state,
                    const uint32_t* poly_len, uint32_t n);
 
-/* Run the selected phases of ONE step (for per-phase parity).  AXG_PHASE_BIN without AXG_PHASE_DIFFUSE first
- * takes the current particle array as the pre-sort array (copy + re-key), so that binning can be checked on
- * positions produced elsewhere.  Synchronises.                                                           */
+/* Run the selected phases of ONE step (for per-phase parity).  AXG_PHASE_BIN bins the output of the step's P1 if one has
+ * run and is still unbinned (in this call or an earlier one); otherwise it takes the current particle array as the
+ * pre-sort array (copy + re-key), so that binning can be checked on positions produced elsewhere.  Synchronises. */
 int axg_step_phase(axg_ctx* ctx, uint32_t phase_mask);
 
 /* Multi-GPU sharding by source: this rank emits only sources with index % world == rank; the

@@ -73,6 +73,8 @@ struct axg_ctx {
     bool b_chunked = false;   // the pre-sort array is in the chunked layout of k_diffuse_chunked (count binning)
     bool kp_pending = false;  // count binning: the last P2 left sorted keys / permutation to be derived on read (k_settle<true>)
     bool cnt_dirty = false;   // P1 has counted into cnt and P2 has not consumed (and re-zeroed) it yet
+    bool p1_pending = false;  // a P1 has run and its output has not been binned yet: the next AXG_PHASE_BIN bins IT
+                              // (the sharded loop enqueues P1 and P2 in separate calls), not a re-keyed copy of A
     void* d_src = nullptr;
     void* d_src_id_prefix = nullptr;
     void* d_src_emit_prefix = nullptr;
@@ -471,11 +473,12 @@ int enqueue_phases(axg_ctx* c, uint32_t mask, Prof& prof, bool overlap = false, 
         c->cnt_dirty = count_mode;
         c->b_chunked = count_mode;
         c->kp_pending = false;  // the records that a replay of k_settle would gather are gone
+        c->p1_pending = true;
     }
     if (mask & AXG_PHASE_BIN) {
         // the previous step's P3 (side stream) still reads cell_lo and the species column that P2 rewrites
         if (overlap && c->adv_pending) cudaStreamWaitEvent(s, c->ev_adv, 0);
-        if (!(mask & AXG_PHASE_DIFFUSE)) {
+        if (!c->p1_pending) {  // no P1 of this step: bin the current array as it stands (harness: given positions)
             zero_cnt_if_dirty();
             prof.mark(AXG_K_EMIT);
             axg_launch_rekey(P, N_SM * 8, s);
@@ -501,6 +504,7 @@ int enqueue_phases(axg_ctx* c, uint32_t mask, Prof& prof, bool overlap = false, 
             axg_launch_reorder(P, N_SM * 8, c->max_particles > AXG_REORDER_WIDE_ABOVE ? 1 : 0, s);
             launches += P.n_pass + 1;
         }
+        c->p1_pending = false;
     }
     cudaStream_t sc = s;  // stream of the cone kernels
     if (overlap) {
@@ -646,6 +650,7 @@ long long enqueue_steps_graph(axg_ctx* c, uint32_t n) {
         cudaStreamWaitEvent(c->stream, c->ev_join, 0);
     }
     c->cnt_dirty = false;
+    c->p1_pending = false;
     c->b_chunked = c->P.bin_mode == AXG_BIN_COUNT_D;
     c->kp_pending = c->b_chunked;
     return launches;
@@ -904,6 +909,7 @@ AXG_API int axg_set_capacity(axg_ctx* c, uint64_t max_particles, uint32_t max_se
         c->particles_allocated = true;
         c->n_B = 0;
         c->kp_pending = false;
+        c->p1_pending = false;
     }
     c->max_particles = max_particles;
     CU(c, cudaMemsetAsync(&((AxgDev*)c->d_dev)->err, 0, sizeof(uint32_t), c->stream));
@@ -943,6 +949,7 @@ AXG_API int axg_load_particles(axg_ctx* c, const float* x, const float* y, const
     CU(c, cudaMemsetAsync(&d->err, 0, sizeof(uint32_t), c->stream));  // a new state: an old capacity hit is history
     CU(c, cudaStreamSynchronize(c->stream));
     c->n_A = n32;
+    c->p1_pending = false;  // ... and an unbinned P1 output belongs to the old state
     c->kp_pending = false;  // A is new: nothing of the last P2 may be replayed
     c->loaded_species_mask = mask;
     return upload_sources(c);

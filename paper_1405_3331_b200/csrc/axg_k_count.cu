@@ -247,7 +247,7 @@ constexpr int SETTLE_ITEMS = 1;  // warp-striped (item i of lane l is slot base 
                                  // 8 blocks per SM 0.188 ms, 2 items 0.198, 4 items / 6 blocks 0.227, 8 items 0.272 --
                                  // the kernel lives on many independent warps in flight, not on ILP inside one
 #ifndef AXG_SETTLE_SORT_MAX
-#define AXG_SETTLE_SORT_MAX 1024
+#define AXG_SETTLE_SORT_MAX 4096
 #endif
 constexpr uint32_t SETTLE_SORT_MAX = AXG_SETTLE_SORT_MAX;
 #ifndef AXG_SETTLE_PREFETCH
@@ -270,35 +270,39 @@ __device__ __forceinline__ void settle_store(const AxgParams& p, uint32_t dst, c
 // One block puts ONE crowded cell (more than SETTLE_INLINE members) into pre-sort order.
 //  m <= SETTLE_SORT_MAX: the members' slot values are sorted in shared memory (bitonic network: O(m log^2 m)), then
 //     gathered in that order.
-//  larger: the members are the valid rows with this key among the physical rows [min, max] of its slot list, and a
-//     row's rank is the number of such rows before it: one pass over that window with a running count (O(window); the
-//     window of a cell is the neighbourhood its particles came from -- the whole array in the worst case).
-// Either way the cost per member no longer grows with the occupancy (D = 0 piles a source's whole emission into one
-// cell: SURVEY.md §8(a) P2b-P2d, reading A-9).
+//  larger: tile by tile -- SETTLE_SORT_MAX members are sorted in shared memory, and EVERY member adds to its rank the
+//     number of entries of that tile below it (a binary search in shared memory); after the last tile a member's rank is
+//     its position.  O(m^2 / SETTLE_SORT_MAX x log): 2e5 members take a few milliseconds of one block instead of the
+//     seconds of the member-by-member loop (D = 0 piles a source's whole emission into one cell: SURVEY.md §8(a) P2b-P2d,
+//     reading A-9).  The ranks accumulate in the cell's own range of skey[final_buf ^ 1], which count binning does not use.
+// The slot value is rotated left by two first: index in the top 30 bits, species in the low 2 -> integer order = order
+// of the pre-sort index.
+__device__ __forceinline__ void settle_bitonic(uint32_t* s_sort, uint32_t n2) {
+    for (uint32_t size = 2u; size <= n2; size <<= 1)
+        for (uint32_t stride = size >> 1; stride > 0u; stride >>= 1) {
+            for (uint32_t t = threadIdx.x; t < (n2 >> 1); t += SETTLE_THREADS) {
+                const uint32_t i = 2u * t - (t & (stride - 1u)), j = i + stride;
+                const uint32_t a = s_sort[i], b = s_sort[j];
+                if ((a > b) == ((i & size) == 0u)) { s_sort[i] = b; s_sort[j] = a; }
+            }
+            __syncthreads();
+        }
+}
+
 template <bool WITH_KP>
-__device__ void settle_big_cell(const AxgParams& p, uint32_t key, uint32_t* s_sort, uint32_t* s_scan) {
+__device__ void settle_big_cell(const AxgParams& p, uint32_t key, uint32_t* s_sort) {
     const uint32_t* __restrict__ slot = p.sidx[p.final_buf ^ 1];
     const uint32_t lo = p.cell_lo[key], hi = p.cell_lo[key + 1u], m = hi - lo;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tid = threadIdx.x;
     if (m <= SETTLE_SORT_MAX) {
         uint32_t n2 = 64u;
         while (n2 < m) n2 <<= 1;
-        // rotate the value left by two: index in the top 30 bits, species in the low 2 -> integer order = index order
         for (uint32_t i = tid; i < n2; i += SETTLE_THREADS) {
-            const uint32_t v = i < m ? slot[lo + i] : 0xffffffffu;
+            const uint32_t v = i < m ? slot[lo + i] : 0u;
             s_sort[i] = i < m ? ((v << 2) | (v >> 30)) : 0xffffffffu;
         }
         __syncthreads();
-        for (uint32_t size = 2u; size <= n2; size <<= 1)
-            for (uint32_t stride = size >> 1; stride > 0u; stride >>= 1) {
-                for (uint32_t t = tid; t < (n2 >> 1); t += SETTLE_THREADS) {
-                    const uint32_t i = 2u * t - (t & (stride - 1u)), j = i + stride;
-                    const uint32_t a = s_sort[i], b = s_sort[j];
-                    const bool up = (i & size) == 0u;
-                    if ((a > b) == up) { s_sort[i] = b; s_sort[j] = a; }
-                }
-                __syncthreads();
-            }
+        settle_bitonic(s_sort, n2);
         for (uint32_t i = tid; i < m; i += SETTLE_THREADS) {
             const uint32_t w = s_sort[i], v = (w >> 2) | (w << 30);
             settle_store<WITH_KP>(p, lo + i, p.Brec[v & AXG_IDX_MASK], v, key);
@@ -306,60 +310,32 @@ __device__ void settle_big_cell(const AxgParams& p, uint32_t key, uint32_t* s_so
         __syncthreads();
         return;
     }
-    // ---- the window of physical rows that holds the members ----
-    uint32_t pmin = 0xffffffffu, pmax = 0u;
-    for (uint32_t i = tid; i < m; i += SETTLE_THREADS) {
-        const uint32_t o = slot[lo + i] & AXG_IDX_MASK;
-        pmin = min(pmin, o);
-        pmax = max(pmax, o);
-    }
-    pmin = __reduce_min_sync(0xffffffffu, pmin);
-    pmax = __reduce_max_sync(0xffffffffu, pmax);
-    if (lane == 0) { s_scan[warp] = pmin; s_scan[8 + warp] = pmax; }
-    __syncthreads();
-    for (int w = 0; w < SETTLE_THREADS / 32; ++w) { pmin = min(pmin, s_scan[w]); pmax = max(pmax, s_scan[8 + w]); }
-    __syncthreads();
-    const uint32_t n_phys = p.dev->n_phys;
-    uint32_t running = 0u;
-    constexpr uint32_t PER = 4u, TILE = SETTLE_THREADS * PER;  // four consecutive rows per thread
-    for (uint32_t t0 = pmin; t0 <= pmax && t0 >= pmin; t0 += TILE) {
-        const uint32_t first = t0 + tid * PER;
-        uint2 w[PER];
-        uint32_t mine = 0u, flags = 0u;
-#pragma unroll
-        for (uint32_t q = 0; q < PER; ++q) {
-            const uint32_t o = first + q;
-            bool ok = o <= pmax && o >= first;
-            if (ok && o < n_phys) ok = (o % AXG_CHUNK) < p.chunk_cnt[o / AXG_CHUNK];  // not a hole (stale words)
-            w[q] = ok ? p.kw[o] : make_uint2(0u, 0u);
-            ok = ok && w[q].x == key;
-            flags |= ok ? (1u << q) : 0u;
-            mine += ok ? 1u : 0u;
+    uint32_t* __restrict__ rank = p.skey[p.final_buf ^ 1] + lo;
+    for (uint32_t i = tid; i < m; i += SETTLE_THREADS) rank[i] = 0u;  // member i is always handled by thread i % 256
+    for (uint32_t t0 = 0u; t0 < m; t0 += SETTLE_SORT_MAX) {
+        const uint32_t tn = min(SETTLE_SORT_MAX, m - t0);
+        for (uint32_t i = tid; i < SETTLE_SORT_MAX; i += SETTLE_THREADS) {
+            const uint32_t v = i < tn ? slot[lo + t0 + i] : 0u;
+            s_sort[i] = i < tn ? ((v << 2) | (v >> 30)) : 0xffffffffu;
         }
-        uint32_t incl = mine;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const uint32_t u = __shfl_up_sync(0xffffffffu, incl, d);
-            if (lane >= d) incl += u;
-        }
-        if (lane == 31) s_scan[warp] = incl;
         __syncthreads();
-        uint32_t before = running, total = 0u;
-        for (int ww = 0; ww < SETTLE_THREADS / 32; ++ww) {
-            const uint32_t c = s_scan[ww];
-            before += ww < warp ? c : 0u;
-            total += c;
-        }
-        uint32_t dst = lo + before + incl - mine;
-#pragma unroll
-        for (uint32_t q = 0; q < PER; ++q)
-            if ((flags >> q) & 1u) {
-                const uint32_t o = first + q;
-                settle_store<WITH_KP>(p, dst++, p.Brec[o], o | (w[q].y & ~AXG_IDX_MASK), key);
+        settle_bitonic(s_sort, SETTLE_SORT_MAX);
+        for (uint32_t i = tid; i < m; i += SETTLE_THREADS) {
+            const uint32_t v = slot[lo + i], x = (v << 2) | (v >> 30);
+            uint32_t a = 0u, b = tn;  // entries of the tile below x
+            while (a < b) {
+                const uint32_t mid = (a + b) >> 1;
+                if (s_sort[mid] < x) a = mid + 1u; else b = mid;
             }
-        running += total;
+            rank[i] += a;
+        }
         __syncthreads();
     }
+    for (uint32_t i = tid; i < m; i += SETTLE_THREADS) {
+        const uint32_t v = slot[lo + i];
+        settle_store<WITH_KP>(p, lo + rank[i], p.Brec[v & AXG_IDX_MASK], v, key);
+    }
+    __syncthreads();
 }
 
 // WITH_KP: also store the sorted keys and the permutation.  Nothing on the path reads them (P1 recomputes the key, P3
@@ -368,7 +344,6 @@ __device__ void settle_big_cell(const AxgParams& p, uint32_t key, uint32_t* s_so
 template <bool WITH_KP>
 __global__ void __launch_bounds__(SETTLE_THREADS, 8) k_settle(const AxgParams p) {
     __shared__ uint32_t s_sort[SETTLE_SORT_MAX];
-    __shared__ uint32_t s_scan[16];
     const uint32_t n = p.dev->n_live;
     const uint32_t* __restrict__ slot = p.sidx[p.final_buf ^ 1];
     const float4* __restrict__ rec = p.Brec;
@@ -424,7 +399,7 @@ __global__ void __launch_bounds__(SETTLE_THREADS, 8) k_settle(const AxgParams p)
     }
     // the crowded cells that k_place listed (a few hundred at C3..C5: the cells next to a source), one block each
     const uint32_t n_big = p.dev->n_big;
-    for (uint32_t w = blockIdx.x; w < n_big; w += gridDim.x) settle_big_cell<WITH_KP>(p, p.big_list[w], s_sort, s_scan);
+    for (uint32_t w = blockIdx.x; w < n_big; w += gridDim.x) settle_big_cell<WITH_KP>(p, p.big_list[w], s_sort);
 }
 
 }  // namespace

@@ -294,9 +294,6 @@ __global__ void __launch_bounds__(DIFF_THREADS, 4) k_diffuse(const AxgParams p) 
 #ifndef AXG_CHUNKED_BLOCKS
 #define AXG_CHUNKED_BLOCKS 4
 #endif
-#ifndef AXG_P1_DYNAMIC
-#define AXG_P1_DYNAMIC 1
-#endif
 #ifndef AXG_P1_STAGES
 #define AXG_P1_STAGES 0   // chunks in flight per warp (bulk-async staging); 0 = per-lane loads held in registers
 #endif
@@ -304,7 +301,9 @@ __global__ void __launch_bounds__(DIFF_THREADS, 4) k_diffuse(const AxgParams p) 
 // 16-byte-aligned run of global memory, so each is ONE 1-D bulk copy (cp.async.bulk -> SASS UBLKCP) whose completion
 // is counted on the stage's mbarrier: the bytes in flight no longer sit in registers behind the scoreboard, and a warp
 // only ever waits for data that was requested two chunks ago.
-constexpr int P1_STAGE_BYTES = 4 * 512 + 128;
+constexpr int CH_ITEMS = AXG_CHUNK_ITEMS;            // rows per lane and trip; one warp trip = one chunk
+constexpr uint32_t CH_COL = AXG_CHUNK * 4u;          // bytes of one 4-byte column of a chunk
+constexpr int P1_STAGE_BYTES = 4 * (int)CH_COL + (int)AXG_CHUNK;
 constexpr int P1_SMEM = AXG_P1_STAGES > 0 ? DIFF_WARPS * AXG_P1_STAGES * P1_STAGE_BYTES
                                           : (int)(AXG_MAX_PASSES * AXG_RADIX * sizeof(uint32_t));  // scratch of emit_and_close
 static_assert(P1_SMEM >= (int)(AXG_MAX_PASSES * AXG_RADIX * sizeof(uint32_t)), "emit_and_close reuses the staging area");
@@ -319,7 +318,7 @@ __global__ void __launch_bounds__(DIFF_THREADS, AXG_CHUNKED_BLOCKS) k_diffuse_ch
     const int tid = threadIdx.x, lane = tid & 31;
     const uint32_t lt = axg_lanemask_lt();
     const AxgRoundKeys rk = axg_round_keys(p.seed_lo, p.seed_hi);
-    static_assert(32 * DIFF_ITEMS == AXG_CHUNK, "one warp trip = one chunk");
+    static_assert(32 * CH_ITEMS == AXG_CHUNK, "one warp trip = one chunk");
     if (tid == 0) s_surv = 0u;
 
     uint32_t mine = 0u;  // survivors of my warp's chunks (lane 0)
@@ -332,11 +331,11 @@ __global__ void __launch_bounds__(DIFF_THREADS, AXG_CHUNKED_BLOCKS) k_diffuse_ch
         const uint32_t bar = my_bar_u32 + 8u * st, dst = my_stage_u32 + (uint32_t)st * P1_STAGE_BYTES;
         const size_t r0 = (size_t)chunk * AXG_CHUNK;  // the arrays are padded: the last chunk may read past n_in
         axg_mbar_expect_tx(bar, P1_STAGE_BYTES);
-        axg_bulk_g2s(dst, p.A.x + r0, 512u, bar);
-        axg_bulk_g2s(dst + 512u, p.A.y + r0, 512u, bar);
-        axg_bulk_g2s(dst + 1024u, p.A.z + r0, 512u, bar);
-        axg_bulk_g2s(dst + 1536u, p.A.id + r0, 512u, bar);
-        axg_bulk_g2s(dst + 2048u, p.A.species + r0, 128u, bar);
+        axg_bulk_g2s(dst, p.A.x + r0, CH_COL, bar);
+        axg_bulk_g2s(dst + CH_COL, p.A.y + r0, CH_COL, bar);
+        axg_bulk_g2s(dst + 2u * CH_COL, p.A.z + r0, CH_COL, bar);
+        axg_bulk_g2s(dst + 3u * CH_COL, p.A.id + r0, CH_COL, bar);
+        axg_bulk_g2s(dst + 4u * CH_COL, p.A.species + r0, AXG_CHUNK, bar);
     };
     if (lane == 0) {
 #pragma unroll
@@ -352,38 +351,27 @@ __global__ void __launch_bounds__(DIFF_THREADS, AXG_CHUNKED_BLOCKS) k_diffuse_ch
 #endif
     __syncthreads();  // s_surv
 
-#if AXG_P1_DYNAMIC && AXG_P1_STAGES == 0
-    // Chunks are handed out by a device ticket, one per warp trip, drawn one trip ahead (its latency hides behind the
-    // arithmetic): SMs differ in speed (distance to the L2 slices, the other die), and with a fixed share per warp the
-    // fast ones idle at the end -- 11 % of the warp slots in the profile of the static loop.
-    uint32_t next_chunk = 0u;
-    if (lane == 0) next_chunk = atomicAdd(&dev->ticket, 1u);
-    next_chunk = __shfl_sync(0xffffffffu, next_chunk, 0);
-    for (uint32_t chunk = next_chunk; chunk < n_chunks; chunk = next_chunk) {
-        if (lane == 0) next_chunk = atomicAdd(&dev->ticket, 1u);
-#else
     for (uint32_t chunk = gw; chunk < n_chunks; chunk += warps_total) {
-#endif
         const uint32_t first = chunk * AXG_CHUNK + lane;
-        float x[DIFF_ITEMS], y[DIFF_ITEMS], z[DIFF_ITEMS];
-        uint32_t id[DIFF_ITEMS], sp[DIFF_ITEMS];
+        float x[CH_ITEMS], y[CH_ITEMS], z[CH_ITEMS];
+        uint32_t id[CH_ITEMS], sp[CH_ITEMS];
 #if AXG_P1_STAGES > 0
         axg_mbar_wait(my_bar_u32 + 8u * st, parity);
         {
             const unsigned char* sb = my_stage + (size_t)st * P1_STAGE_BYTES;
 #pragma unroll
-            for (int i = 0; i < DIFF_ITEMS; ++i) {  // warp-striped rows, as in memory: conflict-free
+            for (int i = 0; i < CH_ITEMS; ++i) {  // warp-striped rows, as in memory: conflict-free
                 const int r = i * 32 + lane;
                 x[i] = reinterpret_cast<const float*>(sb)[r];
-                y[i] = reinterpret_cast<const float*>(sb + 512)[r];
-                z[i] = reinterpret_cast<const float*>(sb + 1024)[r];
-                id[i] = reinterpret_cast<const uint32_t*>(sb + 1536)[r];
-                sp[i] = sb[2048 + r];
+                y[i] = reinterpret_cast<const float*>(sb + CH_COL)[r];
+                z[i] = reinterpret_cast<const float*>(sb + 2 * CH_COL)[r];
+                id[i] = reinterpret_cast<const uint32_t*>(sb + 3 * CH_COL)[r];
+                sp[i] = sb[4 * CH_COL + r];
             }
         }
 #else
 #pragma unroll
-        for (int i = 0; i < DIFF_ITEMS; ++i) {
+        for (int i = 0; i < CH_ITEMS; ++i) {
             const uint32_t g = first + i * 32;
             const bool v = g < n_in;
             // volatile asm: all twenty loads of the chunk are ISSUED here, before the arithmetic of its first row (left
@@ -403,7 +391,7 @@ __global__ void __launch_bounds__(DIFF_THREADS, AXG_CHUNKED_BLOCKS) k_diffuse_ch
         // the divergent part -- ranks and stores -- comes after
         uint32_t alive = 0u;
 #pragma unroll
-        for (int i = 0; i < DIFF_ITEMS; ++i) {
+        for (int i = 0; i < CH_ITEMS; ++i) {
             float z0, z1, z2;
             axg_normals3(id[i], t, 0u, rk, z0, z1, z2);
             x[i] = fmaf(p.sigma, z0, x[i]);
@@ -420,9 +408,9 @@ __global__ void __launch_bounds__(DIFF_THREADS, AXG_CHUNKED_BLOCKS) k_diffuse_ch
         if (++st == AXG_P1_STAGES) { st = 0; parity ^= 1u; }
 #endif
         uint32_t out = chunk * AXG_CHUNK;
-        uint32_t dst[DIFF_ITEMS], arr[DIFF_ITEMS], key[DIFF_ITEMS];
+        uint32_t dst[CH_ITEMS], arr[CH_ITEMS], key[CH_ITEMS];
 #pragma unroll
-        for (int i = 0; i < DIFF_ITEMS; ++i) {  // P1d + P2a
+        for (int i = 0; i < CH_ITEMS; ++i) {  // P1d + P2a
             const bool a = (alive >> i) & 1u;
             const uint32_t b = __ballot_sync(0xffffffffu, a);
             dst[i] = out + __popc(b & lt);
@@ -436,25 +424,19 @@ __global__ void __launch_bounds__(DIFF_THREADS, AXG_CHUNKED_BLOCKS) k_diffuse_ch
             out += __popc(b);
         }
 #pragma unroll
-        for (int i = 0; i < DIFF_ITEMS; ++i)  // the four atomics have been in flight together: one wait, not four
+        for (int i = 0; i < CH_ITEMS; ++i)  // the four atomics have been in flight together: one wait, not four
             if ((alive >> i) & 1u) p.kw[dst[i]] = make_uint2(key[i], arr[i] | (sp[i] << 30));  // species: top two bits
         if (lane == 0) {
             const uint32_t c = out - chunk * AXG_CHUNK;
             p.chunk_cnt[chunk] = c;
             mine += c;
         }
-#if AXG_P1_DYNAMIC && AXG_P1_STAGES == 0
-        next_chunk = __shfl_sync(0xffffffffu, next_chunk, 0);
-#endif
     }
     if (lane == 0 && mine) atomicAdd(&s_surv, mine);
     __syncthreads();
     if (tid == 0 && s_surv) atomicAdd(&dev->n_surv, s_surv);
     if (axg_last_block(dev)) {  // every block's survivors, keys and counts are visible here
-        if (tid == 0) {
-            dev->done = 0u;
-            dev->ticket = 0u;
-        }
+        if (tid == 0) dev->done = 0u;
         __threadfence();
         emit_and_close(p, 1, reinterpret_cast<uint32_t(*)[AXG_RADIX]>(s_raw));
     }

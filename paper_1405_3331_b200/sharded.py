@@ -98,6 +98,10 @@ class ShardedStepper:
         if rest > 0 and self._use_graph and n >= self.GRAPH_MIN_STEPS:
             fp = self.sim.params_fingerprint()
             if self._graph is None or self._graph_fp != fp:
+                # one unit eagerly first: the first collective on a communicator / stream allocates, which a capture
+                # does not allow
+                self._unit(main, True, torch)
+                rest -= 1
                 g = torch.cuda.CUDAGraph()
                 torch.cuda.synchronize()
                 with torch.cuda.graph(g, capture_error_mode="thread_local"):

@@ -158,6 +158,23 @@ def random_particles(seed, n, grid, n_species=2, clustered=True):
     return p[:, 0].copy(), p[:, 1].copy(), p[:, 2].copy(), species, ids
 
 
+def weak_scaled(w: Workload, world: int) -> Workload:
+    """The same config with `world` times the sources (hence particles): new sources of the same species / polarity / rate
+    pattern at fresh seeded positions (4-cell margin), so that under sharding by source every rank owns one config's worth
+    of particles while the cones and the grid stay those of `w` -- the weak-scaling input of `bench.py --scaling weak`."""
+    if world <= 1:
+        return w
+    rng = np.random.default_rng(7000 + w.seed)
+    sources = list(w.sources)
+    for _ in range(world - 1):
+        pos = _uniform_sources(rng, len(w.sources), w.grid, 4.0)
+        sources += [(float(p[0]), float(p[1]), float(p[2]), s[3], s[4], s[5]) for p, s in zip(pos, w.sources)]
+    w.sources = sources
+    w.nominal_live *= world
+    w.notes += " weak-scaled x%d" % world
+    return w
+
+
 BY_NAME = {"C1": c1, "C2": c2, "C3": c3, "C4": c4, "C5": c5}
 
 

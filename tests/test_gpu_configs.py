@@ -115,7 +115,8 @@ def _properties(m, w, sim, key_of):
     cs, ce = sim.read_state("CELL_START"), sim.read_state("CELL_END")
     assert int((ce - cs).sum(dtype=np.int64)) == n
     rng = np.random.default_rng(5)
-    for cell in np.concatenate([rng.integers(0, w.cells, 300), rng.choice(ks, 300)]):
+    for cell in np.concatenate([rng.integers(0, w.cells, 300), rng.choice(ks, 300)]).astype(ks.dtype):
+        # (a key of ks's own dtype: numpy would otherwise convert the whole array for every call)
         lo, hi = np.searchsorted(ks, cell), np.searchsorted(ks, cell, side="right")
         assert (cs[cell], ce[cell]) == ((lo, hi) if hi > lo else (0, 0))
     return a, n

@@ -190,13 +190,13 @@ def test_whole_steps_c1_from_empty(axg):
 def test_crowded_cells_and_d_zero(axg):
     """D = 0 piles a source's whole emission into one cell, and a loaded state may hold any number of particles per cell
     (axg_create accepts D = 0).  Count binning ranks the members of a crowded cell as a whole (k_settle: a block-wide
-    sort up to 1 024 members, a running count over the cell's window of pre-sort rows above that), so the cost per member
-    does not grow with the occupancy: cells of 33, 40, 700, 1 024, 1 025, 5 000 and 200 000 members, bit-exact against
-    the oracle's std::stable_sort in both binning modes, inside a stated time bound."""
+    sort in shared memory up to 4 096 members; above that tile by tile, every member adding up how many entries of each
+    sorted tile lie below it), not member by member: cells of 32, 33, 40, 700, 4 096, 4 097, 5 000 and 200 000 members,
+    bit-exact against the oracle's std::stable_sort in both binning modes, inside a stated time bound."""
     import time
     grid = (16, 12, 10)
     rng = np.random.default_rng(77)
-    sizes = {(3, 3, 3): 200_000, (9, 2, 7): 5_000, (1, 10, 1): 1_025, (12, 5, 5): 1_024, (6, 6, 2): 700, (14, 1, 8): 40,
+    sizes = {(3, 3, 3): 200_000, (9, 2, 7): 5_000, (1, 10, 1): 4_097, (12, 5, 5): 4_096, (6, 6, 2): 700, (14, 1, 8): 40,
              (0, 0, 0): 33, (15, 11, 9): 32}
     pos = [np.asarray(c, np.float64) + rng.uniform(0.0, 1.0, (m, 3)) for c, m in sizes.items()]
     pos.append(rng.uniform(0.0, 1.0, (30_000, 3)) * np.asarray(grid))           # a sparse background
