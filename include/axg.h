@@ -280,6 +280,24 @@ int axg_build_graph(axg_ctx* ctx, int directed);
  * number of edges from root, -1 if v is not reached.  AXG_ESTATE without a graph, AXG_EINVAL for a bad root.        */
 int axg_bfs(axg_ctx* ctx, uint32_t root);
 
+/* The same BFS for callers that may not allocate device memory (code under CUDA graph capture around it, tight serving
+ * loops, harnesses that forbid cudaMalloc): no context, no cudaMalloc / cudaFree / allocating library call -- the scratch
+ * (frontier, updating frontier, visited: one byte per vertex each, and the "frontier not empty" word) is a file-scope
+ * device array of the library, 3 x AXG_BFS_NOALLOC_MAX_VERTICES + 256 bytes (3 MB), which every GPU that loads the library
+ * holds until the process exits.
+ *  va, ea   DEVICE pointers: the adjacency list as AXG_GRAPH_VA / AXG_GRAPH_EA describe it (va[n_vertices + 1] heads,
+ *           ea[va[n_vertices]] neighbours); read only
+ *  level    DEVICE pointer, int32[n_vertices]: written, level from root or -1 (= AXG_BFS_LEVEL)
+ *  stream   a cudaStream_t (NULL: the default stream); the call returns after the stream has been synchronised
+ * All four are owned by the caller.  AXG_EINVAL: a null pointer, n_vertices == 0 or > AXG_BFS_NOALLOC_MAX_VERTICES (use
+ * axg_bfs then), root >= n_vertices; AXG_ECUDA: no current device or a CUDA error; the message is axg_last_error(NULL).
+ * Every call shares the one scratch array, which keeps the last call's contents (each call re-initialises the part it
+ * uses before reading it): calls that overlap on the GPU -- different streams, several host threads -- RACE; serialise
+ * them.  The current CUDA device at the time of the call is the one used.                                          */
+#define AXG_BFS_NOALLOC_MAX_VERTICES 1048576u
+int axg_bfs_noalloc(const uint32_t* va, const uint32_t* ea, uint32_t n_vertices, uint32_t root, int32_t* level,
+                    void* stream);
+
 /* Device pointer (int32[C][AXG_MAX_SPECIES][4] = n,Mx,My,Mz) of the per-cone sensing sums, for the NCCL
  * all-reduce between P3 and P4 when sharded.  *bytes = its size.  Owned by ctx.                           */
 int axg_sense_buffer(axg_ctx* ctx, void** device_ptr, size_t* bytes);

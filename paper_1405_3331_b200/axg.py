@@ -46,7 +46,9 @@ EXPORTS = (
     "axg_get_binning",
     "axg_set_connect", "axg_load_targets", "axg_build_graph", "axg_bfs",
     "axg_enqueue_phase_on", "axg_params_fingerprint",
+    "axg_bfs_noalloc",
 )
+BFS_NOALLOC_MAX_VERTICES = 1 << 20   # include/axg.h AXG_BFS_NOALLOC_MAX_VERTICES
 
 _ALLOC_T = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p)
 _FREE_T = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
@@ -103,6 +105,7 @@ def lib(build=True):
     L.axg_load_targets.argtypes = [vp, vp, u32]
     L.axg_build_graph.argtypes = [vp, C.c_int]
     L.axg_bfs.argtypes = [vp, u32]
+    L.axg_bfs_noalloc.argtypes = [vp, vp, u32, u32, vp, vp]
     L.axg_set_steering.argtypes = [vp, C.c_int, C.c_float, C.c_float]
     L.axg_set_sensing.argtypes = [vp, C.c_int]
     L.axg_set_key_order.argtypes = [vp, C.c_int]
@@ -117,6 +120,15 @@ def lib(build=True):
     L.axg_kernel_times.argtypes = [vp, vp]
     _lib = L
     return L
+
+
+def bfs_noalloc(va_ptr, ea_ptr, n_vertices, root, level_ptr, cuda_stream=0):
+    """axg_bfs_noalloc: BFS over a device-resident adjacency list with the library's fixed scratch array; allocates
+    nothing.  All pointers are DEVICE addresses (ints); `level_ptr` receives int32[n_vertices]."""
+    L = lib()
+    rc = L.axg_bfs_noalloc(int(va_ptr), int(ea_ptr), int(n_vertices), int(root), int(level_ptr), int(cuda_stream or 0))
+    if rc:
+        raise AxgError(rc, L.axg_last_error(None).decode())
 
 
 def use_torch_allocator():

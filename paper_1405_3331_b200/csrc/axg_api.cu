@@ -34,6 +34,9 @@ constexpr uint64_t AXG_REORDER_WIDE_ABOVE = 32ull << 20;
 
 }  // namespace
 
+// the message of a failing call that has no context (axg_create, axg_bfs_noalloc): what axg_last_error(NULL) returns
+void axg_set_global_error(const char* msg) { g_create_err = msg ? msg : ""; }
+
 struct axg_ctx {
     axg_grid grid;
     float D, radius, speed, noise;

@@ -297,3 +297,81 @@ void axg_launch_bfs_level(const AxgGraph& g, cudaStream_t s) {
     k_bfs_expand<<<grid_for(g.n), G_THREADS, 0, s>>>(g);
     k_bfs_advance<<<grid_for(g.n), G_THREADS, 0, s>>>(g);
 }
+
+// ---- the BFS for callers that may not allocate (include/axg.h axg_bfs_noalloc) ---------------------------------------------
+// Same kernels, same algorithm (reading A-30) as axg_bfs; what differs is where the scratch lives: the frontier, the
+// updating frontier, the visited flags (one byte per vertex each) and the "frontier not empty" word sit in ONE file-scope
+// device array of fixed size instead of buffers taken from the allocator.  Every GPU that loads the library holds these
+// 3 MB + 256 B until exit.  All calls share the array and it keeps the last call's contents: k_bfs_init rewrites all four
+// regions for the vertices of THIS call before anything reads them, and two calls that overlap on the GPU (different
+// streams, or two host threads) race on it.
+#include "../../include/axg.h"
+
+void axg_set_global_error(const char* msg);  // axg_api.cu: the message axg_last_error(NULL) returns
+
+namespace {
+
+constexpr uint32_t NOALLOC_MAX_VERTICES = AXG_BFS_NOALLOC_MAX_VERTICES;
+constexpr size_t NOALLOC_FLAG_AT = 3 * (size_t)NOALLOC_MAX_VERTICES;  // a multiple of 256
+static __device__ __align__(256) unsigned char g_bfs_scratch[NOALLOC_FLAG_AT + 256];
+
+// In host code `g_bfs_scratch` is a host-side stand-in for the symbol, not a device address: the address is asked of the
+// runtime once per device, with that device current, and cached.
+constexpr int NOALLOC_MAX_DEVICES = 64;
+unsigned char* g_bfs_scratch_dev[NOALLOC_MAX_DEVICES] = {nullptr};
+
+int noalloc_fail(int code, const char* msg) {
+    axg_set_global_error(msg);
+    return code;
+}
+
+}  // namespace
+
+extern "C" __attribute__((visibility("default"))) int axg_bfs_noalloc(const uint32_t* va, const uint32_t* ea,
+                                                                      uint32_t n_vertices, uint32_t root, int32_t* level,
+                                                                      void* stream) {
+    if (!va || !ea || !level) return noalloc_fail(AXG_EINVAL, "axg_bfs_noalloc: null argument");
+    if (n_vertices == 0) return noalloc_fail(AXG_EINVAL, "axg_bfs_noalloc: empty graph");
+    if (n_vertices > NOALLOC_MAX_VERTICES)
+        return noalloc_fail(AXG_EINVAL, "axg_bfs_noalloc: more vertices than AXG_BFS_NOALLOC_MAX_VERTICES (2^20): the "
+                                        "scratch array is fixed; use axg_bfs");
+    if (root >= n_vertices) return noalloc_fail(AXG_EINVAL, "axg_bfs_noalloc: root out of range");
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= NOALLOC_MAX_DEVICES) {
+        cudaGetLastError();
+        return noalloc_fail(AXG_ECUDA, "axg_bfs_noalloc: no current CUDA device");
+    }
+    if (!g_bfs_scratch_dev[dev]) {
+        void* ptr = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&ptr, g_bfs_scratch);
+        if (e != cudaSuccess || !ptr) {
+            cudaGetLastError();
+            return noalloc_fail(AXG_ECUDA, "axg_bfs_noalloc: cudaGetSymbolAddress failed");
+        }
+        g_bfs_scratch_dev[dev] = static_cast<unsigned char*>(ptr);
+    }
+    unsigned char* const scratch = g_bfs_scratch_dev[dev];
+    cudaStream_t s = (cudaStream_t)stream;
+    AxgGraph g = {};
+    g.n = n_vertices;
+    g.Va = const_cast<uint32_t*>(va);  // read only by the BFS kernels
+    g.Ea = const_cast<uint32_t*>(ea);
+    g.C = level;
+    g.F = scratch;
+    g.Fu = scratch + NOALLOC_MAX_VERTICES;
+    g.X = scratch + 2 * (size_t)NOALLOC_MAX_VERTICES;
+    g.flag = reinterpret_cast<uint32_t*>(scratch + NOALLOC_FLAG_AT);
+    k_bfs_init<<<grid_for(n_vertices), G_THREADS, 0, s>>>(g, root);  // clears F / Fu / X / C of this call's vertices
+    for (uint32_t lv = 0; lv <= n_vertices; ++lv) {  // "repeated until frontier is empty"
+        uint32_t more = 0;
+        cudaError_t e = cudaMemsetAsync(g.flag, 0, 4, s);
+        k_bfs_expand<<<grid_for(n_vertices), G_THREADS, 0, s>>>(g);
+        k_bfs_advance<<<grid_for(n_vertices), G_THREADS, 0, s>>>(g);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(&more, g.flag, 4, cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        if (e == cudaSuccess) e = cudaGetLastError();
+        if (e != cudaSuccess) return noalloc_fail(AXG_ECUDA, cudaGetErrorString(e));
+        if (!more) break;
+    }
+    return AXG_OK;
+}
