@@ -41,13 +41,15 @@ HBM_FALLBACK_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md "FALLBACK"
 NOMINAL_GBS = 8000.0          # north_star's "~8 TB/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the `ncu --set full` capture
 # summarised in profiles/ (a capture is not repeatable inside a timed run, so it is a recorded number).
-TRAFFIC_NCU = {   # (workload, kernel) -> bytes per launch; profiles/r01_summary.md, r01c_summary.md
-    ("C3", "k_diffuse_chunked"): 753.7e6, ("C3", "k_diffuse"): 578.9e6, ("C3", "k_settle"): 652.7e6,
-    ("C3", "k_place"): 248.8e6, ("C3", "k_cell_scan2"): 172.6e6, ("C3", "k_sort_pass"): 203.7e6,
+TRAFFIC_NCU = {   # (workload, kernel) -> bytes per launch; profiles/r02_summary.md (radix kernels: r01_summary.md)
+    ("C3", "k_diffuse_chunked"): 754.8e6, ("C3", "k_diffuse"): 578.9e6, ("C3", "k_settle"): 654.7e6,
+    ("C3", "k_place"): 247.1e6, ("C3", "k_cell_scan2"): 175.0e6, ("C3", "k_sort_pass"): 203.7e6,
     ("C3", "k_reorder"): 740.8e6,
+    ("C4", "k_diffuse_chunked"): 3718.3e6, ("C4", "k_settle"): 2855.0e6, ("C4", "k_place"): 1255.4e6,
+    ("C4", "k_cell_scan2"): 2088.0e6,
 }
 # the same capture summed over the kernels of one step (count binning: P1 + scan + place + settle + sense + advance)
-STEP_TRAFFIC_NCU = {("C3", "count"): 1832.0e6}
+STEP_TRAFFIC_NCU = {("C3", "count"): 1836.0e6, ("C4", "count"): 9920.0e6}
 
 
 def log(*a):
@@ -217,7 +219,7 @@ class ClockSampler:
 # ---------------------------------------------------------------------------------------------------------------
 # the oracle on host cores (cpu_baseline leg and --impl reference arm): the only places bench.py runs oracle/
 # ---------------------------------------------------------------------------------------------------------------
-def time_oracle(w, n_sample, steps, warmup, seed=4242):
+def time_oracle(w, n_sample, steps, warmup, seed=4242, want_n_end=False):
     """Particle-steps/s of the CPU oracle (single thread, as it stands) on `w` with a synthetic steady-state-shaped
     population of n_sample particles (workloads.synthetic_population).  Returns (value, seconds, particle_steps)."""
     from oracle import axo
@@ -238,7 +240,10 @@ def time_oracle(w, n_sample, steps, warmup, seed=4242):
         o.step(1)
         secs += time.perf_counter() - t0
         psteps += n_in
+    n_end = o.counters()["n_live"]
     o.close()
+    if want_n_end:
+        return psteps / max(secs, 1e-12), secs, psteps, n_end
     return psteps / max(secs, 1e-12), secs, psteps
 
 
@@ -258,7 +263,7 @@ def run_reference(args, w):
     """--impl reference: the oracle, timed on host cores; each step a bounded sample of the workload."""
     budget = float(os.environ.get("AXG_REFERENCE_BUDGET_S", "60"))
     n = oracle_sample_size(w, budget, args.steps + args.warmup)
-    value, secs, psteps = time_oracle(w, n, args.steps, args.warmup)
+    value, secs, psteps, n_end = time_oracle(w, n, args.steps, args.warmup, want_n_end=True)
     sample = "%d of the workload's ~%d particles (synthetic steady-state-shaped population), all %d cones, %d steps" % (
         n, w.nominal_live, len(w.neurons), args.steps)
     line = {
@@ -266,7 +271,8 @@ def run_reference(args, w):
         "warmup": args.warmup, "ms_per_step": 1e3 * secs / max(args.steps, 1), "higher_is_better": True,
         "scaling": "strong" if args.gpus > 1 else "weak", "vs_baseline": None, "dtype": "f32+u32 (oracle: f64 Box-Muller)",
         "data": "synthetic", "config": {"workload": w.name, "grid": list(w.grid), "cones": int(len(w.neurons)),
-                                        "sources": len(w.sources), "sample_particles": n},
+                                        "sources": len(w.sources), "n_live_start": n, "n_live_end": n_end,
+                                        "sample_particles": n},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,

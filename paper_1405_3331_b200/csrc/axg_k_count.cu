@@ -234,7 +234,7 @@ __global__ void __launch_bounds__(PLACE_THREADS) k_place(const AxgParams p) {
     // returned every row's arrival rank inside its cell (kw.y), in the arbitrary order of the atomics.
     for (uint32_t o = blockIdx.x * PLACE_THREADS + threadIdx.x; o < n_pp; o += gridDim.x * PLACE_THREADS) {
         if (o < n_phys && (o % AXG_CHUNK) >= __ldg(p.chunk_cnt + o / AXG_CHUNK)) continue;  // a hole
-        const uint2 w = __ldg(p.kw + o);  // key, arrival rank | species << 30: one 8-byte load
+        const uint2 w = axg_ld_stream(p.kw + o);  // key, arrival rank | species << 30: one 8-byte load
         const uint32_t arr = w.y & AXG_IDX_MASK;
         slot[__ldg(cell_lo + w.x) + arr] = o | (w.y & ~AXG_IDX_MASK);
         if (arr == SETTLE_INLINE) p.big_list[atomicAdd(&p.dev->n_big, 1u)] = w.x;  // at most n_live / 33 entries
@@ -256,11 +256,11 @@ constexpr uint32_t SETTLE_SORT_MAX = AXG_SETTLE_SORT_MAX;
 
 template <bool WITH_KP>
 __device__ __forceinline__ void settle_store(const AxgParams& p, uint32_t dst, const float4& r, uint32_t v, uint32_t k) {
-    p.A.x[dst] = r.x;
-    p.A.y[dst] = r.y;
-    p.A.z[dst] = r.z;
-    p.A.id[dst] = __float_as_uint(r.w);
-    p.A.species[dst] = (uint8_t)(v >> 30);
+    axg_st_stream(p.A.x + dst, r.x);
+    axg_st_stream(p.A.y + dst, r.y);
+    axg_st_stream(p.A.z + dst, r.z);
+    axg_st_stream(p.A.id + dst, __float_as_uint(r.w));
+    axg_st_stream(reinterpret_cast<unsigned char*>(p.A.species) + dst, (unsigned char)(v >> 30));
     if (WITH_KP) {
         p.skey[p.final_buf][dst] = k;
         p.sidx[p.final_buf][dst] = v;
@@ -376,7 +376,7 @@ __global__ void __launch_bounds__(SETTLE_THREADS, 8) k_settle(const AxgParams p)
 #pragma unroll
         for (int i = 0; i < SETTLE_ITEMS; ++i) {
             const uint32_t j = base + 32u * i + lane;
-            v[i] = (j < n) ? __ldg(slot + j) : 0u;
+            v[i] = (j < n) ? axg_ld_stream(slot + j) : 0u;
         }
 #pragma unroll
         for (int i = 0; i < SETTLE_ITEMS; ++i) {

@@ -379,11 +379,19 @@ __global__ void __launch_bounds__(DIFF_THREADS, AXG_CHUNKED_BLOCKS) k_diffuse_ch
             // and every row then pays a full memory latency: 42 % of the stall samples)
             x[i] = -1.0f; y[i] = -1.0f; z[i] = -1.0f; id[i] = 0u; sp[i] = 0u;
             if (v) {
+#if AXG_CS
+                asm volatile("ld.global.cs.f32 %0, [%1];" : "=f"(x[i]) : "l"(p.A.x + g) : "memory");
+                asm volatile("ld.global.cs.f32 %0, [%1];" : "=f"(y[i]) : "l"(p.A.y + g) : "memory");
+                asm volatile("ld.global.cs.f32 %0, [%1];" : "=f"(z[i]) : "l"(p.A.z + g) : "memory");
+                asm volatile("ld.global.cs.u32 %0, [%1];" : "=r"(id[i]) : "l"(p.A.id + g) : "memory");
+                asm volatile("ld.global.cs.u8 %0, [%1];" : "=r"(sp[i]) : "l"(p.A.species + g) : "memory");
+#else
                 asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(x[i]) : "l"(p.A.x + g) : "memory");
                 asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(y[i]) : "l"(p.A.y + g) : "memory");
                 asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(z[i]) : "l"(p.A.z + g) : "memory");
                 asm volatile("ld.global.nc.u32 %0, [%1];" : "=r"(id[i]) : "l"(p.A.id + g) : "memory");
                 asm volatile("ld.global.nc.u8 %0, [%1];" : "=r"(sp[i]) : "l"(p.A.species + g) : "memory");
+#endif
             }
         }
 #endif
@@ -419,13 +427,13 @@ __global__ void __launch_bounds__(DIFF_THREADS, AXG_CHUNKED_BLOCKS) k_diffuse_ch
             if (a) {
                 key[i] = axg_cell_key(p, x[i], y[i], z[i]);
                 arr[i] = atomicAdd(p.cnt + key[i], 1u);  // old count = arrival rank inside the cell (see tally)
-                p.Brec[dst[i]] = make_float4(x[i], y[i], z[i], __uint_as_float(id[i]));
+                axg_st_stream(p.Brec + dst[i], make_float4(x[i], y[i], z[i], __uint_as_float(id[i])));
             }
             out += __popc(b);
         }
 #pragma unroll
         for (int i = 0; i < CH_ITEMS; ++i)  // the four atomics have been in flight together: one wait, not four
-            if ((alive >> i) & 1u) p.kw[dst[i]] = make_uint2(key[i], arr[i] | (sp[i] << 30));  // species: top two bits
+            if ((alive >> i) & 1u) axg_st_stream(p.kw + dst[i], make_uint2(key[i], arr[i] | (sp[i] << 30)));  // species: top two bits
         if (lane == 0) {
             const uint32_t c = out - chunk * AXG_CHUNK;
             p.chunk_cnt[chunk] = c;
