@@ -217,6 +217,10 @@ int alloc_fixed(axg_ctx* c) {
     P.cell_lo = (uint32_t*)c->d_cell_lo;
     P.nx = c->grid.nx; P.ny = c->grid.ny; P.nz = c->grid.nz; P.cells = (uint32_t)c->cells();
     P.key_order = c->key_order; P.nbx = (uint32_t)c->nbx(); P.nby = (uint32_t)c->nby();
+    {   // streaming hints where the per-cell arrays (4 B x cells each) are beyond the L2 (126 MB): C4, C5; not C1..C3
+        const char* e = std::getenv("AXG_STREAM_HINT");  // 0 / 1 overrides (measurements)
+        P.cs = e ? (e[0] == '1') : (c->cells() * sizeof(uint32_t) > (size_t)256 << 20);
+    }
     {   // the phases of the Z-order bit rotation (reading A-31)
         const int nb[3] = {axg_ctx::axis_bits(c->grid.nx), axg_ctx::axis_bits(c->grid.ny), axg_ctx::axis_bits(c->grid.nz)};
         const int m3 = std::min(nb[0], std::min(nb[1], nb[2]));

@@ -223,6 +223,7 @@ constexpr int PLACE_THREADS = 256;
 // exactly SETTLE_INLINE exists once in every cell with more than SETTLE_INLINE members.
 constexpr uint32_t SETTLE_INLINE = 32u;
 
+template <bool CS>
 __global__ void __launch_bounds__(PLACE_THREADS) k_place(const AxgParams p) {
     // B is in the chunked layout of k_diffuse_chunked: every physical row below n_pp is visited, the holes at the end
     // of each chunk are skipped, and the slot value is the PHYSICAL row (it orders the rows like the dense index)
@@ -234,7 +235,7 @@ __global__ void __launch_bounds__(PLACE_THREADS) k_place(const AxgParams p) {
     // returned every row's arrival rank inside its cell (kw.y), in the arbitrary order of the atomics.
     for (uint32_t o = blockIdx.x * PLACE_THREADS + threadIdx.x; o < n_pp; o += gridDim.x * PLACE_THREADS) {
         if (o < n_phys && (o % AXG_CHUNK) >= __ldg(p.chunk_cnt + o / AXG_CHUNK)) continue;  // a hole
-        const uint2 w = axg_ld_stream(p.kw + o);  // key, arrival rank | species << 30: one 8-byte load
+        const uint2 w = axg_ld_stream<CS>(p.kw + o);  // key, arrival rank | species << 30: one 8-byte load
         const uint32_t arr = w.y & AXG_IDX_MASK;
         slot[__ldg(cell_lo + w.x) + arr] = o | (w.y & ~AXG_IDX_MASK);
         if (arr == SETTLE_INLINE) p.big_list[atomicAdd(&p.dev->n_big, 1u)] = w.x;  // at most n_live / 33 entries
@@ -256,11 +257,11 @@ constexpr uint32_t SETTLE_SORT_MAX = AXG_SETTLE_SORT_MAX;
 
 template <bool WITH_KP>
 __device__ __forceinline__ void settle_store(const AxgParams& p, uint32_t dst, const float4& r, uint32_t v, uint32_t k) {
-    axg_st_stream(p.A.x + dst, r.x);
-    axg_st_stream(p.A.y + dst, r.y);
-    axg_st_stream(p.A.z + dst, r.z);
-    axg_st_stream(p.A.id + dst, __float_as_uint(r.w));
-    axg_st_stream(reinterpret_cast<unsigned char*>(p.A.species) + dst, (unsigned char)(v >> 30));
+    p.A.x[dst] = r.x;  // (streaming hints measured on these stores and on the slot loads: no gain at C4 / C5)
+    p.A.y[dst] = r.y;
+    p.A.z[dst] = r.z;
+    p.A.id[dst] = __float_as_uint(r.w);
+    p.A.species[dst] = (uint8_t)(v >> 30);
     if (WITH_KP) {
         p.skey[p.final_buf][dst] = k;
         p.sidx[p.final_buf][dst] = v;
@@ -376,7 +377,7 @@ __global__ void __launch_bounds__(SETTLE_THREADS, 8) k_settle(const AxgParams p)
 #pragma unroll
         for (int i = 0; i < SETTLE_ITEMS; ++i) {
             const uint32_t j = base + 32u * i + lane;
-            v[i] = (j < n) ? axg_ld_stream(slot + j) : 0u;
+            v[i] = (j < n) ? __ldg(slot + j) : 0u;
         }
 #pragma unroll
         for (int i = 0; i < SETTLE_ITEMS; ++i) {
@@ -411,6 +412,8 @@ void axg_launch_cell_scan(const AxgParams& p, int grid, cudaStream_t s) {
         cudaGetLastError();
         resident = 0;
     }
+    // (The chained single-pass kernel reads cnt once instead of twice -- 12 instead of 16 B per cell -- but loses also where
+    // the scan is DRAM-bound: C4 0.518 vs 0.355 ms, C5 1.03 vs 0.69 ms; the two-phase kernel runs at the copy roofline.)
     if (resident >= SCAN2_BLOCKS_PER_SM) {
         // cooperative launch: the driver schedules all blocks of the grid together or not at all, so the grid barrier
         // cannot deadlock against another context's kernels
@@ -429,7 +432,9 @@ void axg_launch_cell_scan(const AxgParams& p, int grid, cudaStream_t s) {
     }
     k_cell_scan<<<grid, SCAN_THREADS, 0, s>>>(p);
 }
-void axg_launch_place(const AxgParams& p, int grid, cudaStream_t s) { k_place<<<grid, PLACE_THREADS, 0, s>>>(p); }
+void axg_launch_place(const AxgParams& p, int grid, cudaStream_t s) {
+    if (p.cs) k_place<true><<<grid, PLACE_THREADS, 0, s>>>(p); else k_place<false><<<grid, PLACE_THREADS, 0, s>>>(p);
+}
 void axg_launch_settle(const AxgParams& p, int grid, int with_keys_perm, cudaStream_t s) {
     if (with_keys_perm) k_settle<true><<<grid, SETTLE_THREADS, 0, s>>>(p);
     else k_settle<false><<<grid, SETTLE_THREADS, 0, s>>>(p);

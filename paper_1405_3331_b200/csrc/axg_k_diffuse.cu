@@ -308,6 +308,7 @@ constexpr int P1_SMEM = AXG_P1_STAGES > 0 ? DIFF_WARPS * AXG_P1_STAGES * P1_STAG
                                           : (int)(AXG_MAX_PASSES * AXG_RADIX * sizeof(uint32_t));  // scratch of emit_and_close
 static_assert(P1_SMEM >= (int)(AXG_MAX_PASSES * AXG_RADIX * sizeof(uint32_t)), "emit_and_close reuses the staging area");
 
+template <bool CS>
 __global__ void __launch_bounds__(DIFF_THREADS, AXG_CHUNKED_BLOCKS) k_diffuse_chunked(const AxgParams p) {
     extern __shared__ __align__(128) unsigned char s_raw[];
     __shared__ __align__(8) unsigned long long s_bar[DIFF_WARPS][AXG_P1_STAGES > 0 ? AXG_P1_STAGES : 1];
@@ -379,19 +380,19 @@ __global__ void __launch_bounds__(DIFF_THREADS, AXG_CHUNKED_BLOCKS) k_diffuse_ch
             // and every row then pays a full memory latency: 42 % of the stall samples)
             x[i] = -1.0f; y[i] = -1.0f; z[i] = -1.0f; id[i] = 0u; sp[i] = 0u;
             if (v) {
-#if AXG_CS
-                asm volatile("ld.global.cs.f32 %0, [%1];" : "=f"(x[i]) : "l"(p.A.x + g) : "memory");
-                asm volatile("ld.global.cs.f32 %0, [%1];" : "=f"(y[i]) : "l"(p.A.y + g) : "memory");
-                asm volatile("ld.global.cs.f32 %0, [%1];" : "=f"(z[i]) : "l"(p.A.z + g) : "memory");
-                asm volatile("ld.global.cs.u32 %0, [%1];" : "=r"(id[i]) : "l"(p.A.id + g) : "memory");
-                asm volatile("ld.global.cs.u8 %0, [%1];" : "=r"(sp[i]) : "l"(p.A.species + g) : "memory");
-#else
-                asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(x[i]) : "l"(p.A.x + g) : "memory");
-                asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(y[i]) : "l"(p.A.y + g) : "memory");
-                asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(z[i]) : "l"(p.A.z + g) : "memory");
-                asm volatile("ld.global.nc.u32 %0, [%1];" : "=r"(id[i]) : "l"(p.A.id + g) : "memory");
-                asm volatile("ld.global.nc.u8 %0, [%1];" : "=r"(sp[i]) : "l"(p.A.species + g) : "memory");
-#endif
+                if constexpr (CS) {
+                    asm volatile("ld.global.cs.f32 %0, [%1];" : "=f"(x[i]) : "l"(p.A.x + g) : "memory");
+                    asm volatile("ld.global.cs.f32 %0, [%1];" : "=f"(y[i]) : "l"(p.A.y + g) : "memory");
+                    asm volatile("ld.global.cs.f32 %0, [%1];" : "=f"(z[i]) : "l"(p.A.z + g) : "memory");
+                    asm volatile("ld.global.cs.u32 %0, [%1];" : "=r"(id[i]) : "l"(p.A.id + g) : "memory");
+                    asm volatile("ld.global.cs.u8 %0, [%1];" : "=r"(sp[i]) : "l"(p.A.species + g) : "memory");
+                } else {
+                    asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(x[i]) : "l"(p.A.x + g) : "memory");
+                    asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(y[i]) : "l"(p.A.y + g) : "memory");
+                    asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(z[i]) : "l"(p.A.z + g) : "memory");
+                    asm volatile("ld.global.nc.u32 %0, [%1];" : "=r"(id[i]) : "l"(p.A.id + g) : "memory");
+                    asm volatile("ld.global.nc.u8 %0, [%1];" : "=r"(sp[i]) : "l"(p.A.species + g) : "memory");
+                }
             }
         }
 #endif
@@ -427,13 +428,13 @@ __global__ void __launch_bounds__(DIFF_THREADS, AXG_CHUNKED_BLOCKS) k_diffuse_ch
             if (a) {
                 key[i] = axg_cell_key(p, x[i], y[i], z[i]);
                 arr[i] = atomicAdd(p.cnt + key[i], 1u);  // old count = arrival rank inside the cell (see tally)
-                axg_st_stream(p.Brec + dst[i], make_float4(x[i], y[i], z[i], __uint_as_float(id[i])));
+                axg_st_stream<CS>(p.Brec + dst[i], make_float4(x[i], y[i], z[i], __uint_as_float(id[i])));
             }
             out += __popc(b);
         }
 #pragma unroll
         for (int i = 0; i < CH_ITEMS; ++i)  // the four atomics have been in flight together: one wait, not four
-            if ((alive >> i) & 1u) axg_st_stream(p.kw + dst[i], make_uint2(key[i], arr[i] | (sp[i] << 30)));  // species: top two bits
+            if ((alive >> i) & 1u) axg_st_stream<CS>(p.kw + dst[i], make_uint2(key[i], arr[i] | (sp[i] << 30)));  // species: top two bits
         if (lane == 0) {
             const uint32_t c = out - chunk * AXG_CHUNK;
             p.chunk_cnt[chunk] = c;
@@ -494,15 +495,12 @@ void axg_launch_diffuse(const AxgParams& p, int grid, cudaStream_t s) {
     if (p.bin_mode == AXG_BIN_COUNT_D) {
         static bool attr_set = false;  // dynamic shared memory above 48 KB needs the opt-in once per process
         if (!attr_set) {
-            cudaFuncSetAttribute(k_diffuse_chunked, cudaFuncAttributeMaxDynamicSharedMemorySize, P1_SMEM);
+            cudaFuncSetAttribute(k_diffuse_chunked<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, P1_SMEM);
+            cudaFuncSetAttribute(k_diffuse_chunked<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, P1_SMEM);
             attr_set = true;
         }
-        cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3(148 * AXG_CHUNKED_BLOCKS);
-        cfg.blockDim = dim3(DIFF_THREADS);
-        cfg.dynamicSmemBytes = P1_SMEM;
-        cfg.stream = s;
-        cudaLaunchKernelEx(&cfg, k_diffuse_chunked, p);
+        if (p.cs) k_diffuse_chunked<true><<<148 * AXG_CHUNKED_BLOCKS, DIFF_THREADS, P1_SMEM, s>>>(p);
+        else k_diffuse_chunked<false><<<148 * AXG_CHUNKED_BLOCKS, DIFF_THREADS, P1_SMEM, s>>>(p);
     } else {
         k_diffuse<<<grid, DIFF_THREADS, 0, s>>>(p);
     }

@@ -165,11 +165,12 @@ def weak_scaled(w: Workload, world: int) -> Workload:
     if world <= 1:
         return w
     rng = np.random.default_rng(7000 + w.seed)
-    sources = list(w.sources)
+    copies = [list(w.sources)]
     for _ in range(world - 1):
         pos = _uniform_sources(rng, len(w.sources), w.grid, 4.0)
-        sources += [(float(p[0]), float(p[1]), float(p[2]), s[3], s[4], s[5]) for p, s in zip(pos, w.sources)]
-    w.sources = sources
+        copies.append([(float(p[0]), float(p[1]), float(p[2]), s[3], s[4], s[5]) for p, s in zip(pos, w.sources)])
+    # rank r owns the sources with index % world == r (axg_set_shard): interleave, so that rank r owns exactly copy r
+    w.sources = [copies[r][i] for i in range(len(copies[0])) for r in range(world)]
     w.nominal_live *= world
     w.notes += " weak-scaled x%d" % world
     return w

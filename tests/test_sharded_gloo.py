@@ -131,3 +131,26 @@ def test_owned_sources_partition():
     for world in (1, 2, 3, 8):
         seen = sorted(s for r in range(world) for s in sharded.owned_sources(13, r, world))
         assert seen == list(range(13))
+
+
+def test_weak_scaled_workload_gives_every_rank_one_configs_worth_of_sources():
+    """bench.py --scaling weak: `world` times the sources (same species / polarity / rate pattern, new seeded positions
+    inside the 4-cell margin), cones and grid unchanged, so that sharding by source leaves every rank with the source
+    count -- hence the particle count -- of the 1-GPU config."""
+    from paper_1405_3331_b200 import sharded, workloads as W
+    base = W.c3()
+    for world in (1, 2, 8):
+        w = W.weak_scaled(W.c3(), world)
+        assert len(w.sources) == world * len(base.sources) and w.grid == base.grid
+        assert np.array_equal(w.neurons, base.neurons) and w.max_particles == base.max_particles
+        assert w.sources[::world] == base.sources                                        # rank 0 owns the config's own
+        for r in range(world):
+            own = [w.sources[s] for s in sharded.owned_sources(len(w.sources), r, world)]
+            assert len(own) == len(base.sources)
+            assert sum(s[5] for s in own) == base.emitted_per_step
+            assert sorted(s[3] for s in own) == sorted(s[3] for s in base.sources)      # same species mix per rank
+        for s in w.sources:
+            assert all(4.0 <= s[a] <= w.grid[a] - 4.0 for a in range(3))
+        pol = {}
+        for s in w.sources:
+            assert pol.setdefault(s[3], s[4]) == s[4]                                    # one polarity per species
