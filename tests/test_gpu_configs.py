@@ -242,14 +242,11 @@ def test_c5_properties_and_samples(c5, mode):
 
 def test_c5_diffuse_and_bin_against_the_oracle(c5):
     """P1 + P2 of one C5 step against the oracle (its P3..P5 over 10^6 cones are covered at C4 / C3 size and by the
-    sampled cones above).  Needs ~40 GB of host memory for the two sides' arrays: skipped, with the reason, below that."""
-    import os
+    sampled cones above): 2.3e8 particles by id within tolerance, then keys, permutation, cellStart / cellEnd and the
+    reordered columns bit for bit.  About 70 s of host time (profiles/r02_c5_oracle_test.txt).  Needs ~40 GB of host memory
+    for the two sides' arrays: skipped, with the reason, below that."""
     import psutil
     m, w, sim = c5
-    if os.environ.get("AXG_TEST_C5_ORACLE", "0") != "1":
-        pytest.skip("not run by default: one oracle step over 2.3e8 particles (double-precision Box-Muller, "
-                    "std::stable_sort) plus the numpy comparisons take ~10 min of host time, more than the whole GPU "
-                    "suite may use; run with AXG_TEST_C5_ORACLE=1 (result of this round: profiles/r02_summary.md)")
     avail = psutil.virtual_memory().available
     if avail < 48 << 30:
         pytest.skip("not run: %.0f GB of host memory available, the two sides' C5 arrays need ~40 GB" % (avail / 2**30))
