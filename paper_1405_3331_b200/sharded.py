@@ -55,7 +55,8 @@ class ShardedStepper:
         sim.set_shard(self.rank, self.world)
         self._exchange = exchange(sim) if self.world > 1 else (lambda: None)
         self._overlap = hasattr(sim, "enqueue_phase_on") if overlap is None else bool(overlap)
-        self._use_graph = bool(graph)
+        import os
+        self._use_graph = bool(graph) and os.environ.get("AXG_SHARDED_GRAPH", "1") != "0"
         self._side = None
         self._graph = None
         self._graph_fp = None
@@ -102,13 +103,28 @@ class ShardedStepper:
                 # does not allow
                 self._unit(main, True, torch)
                 rest -= 1
-                g = torch.cuda.CUDAGraph()
-                torch.cuda.synchronize()
-                with torch.cuda.graph(g, capture_error_mode="thread_local"):
-                    self._unit(torch.cuda.current_stream(), True, torch)
-                self._graph, self._graph_fp = g, fp
-            for _ in range(rest):
-                self._graph.replay()
+                try:
+                    g = torch.cuda.CUDAGraph()
+                    torch.cuda.synchronize()
+                    with torch.cuda.graph(g, capture_error_mode="thread_local"):
+                        self._unit(torch.cuda.current_stream(), True, torch)
+                    self._graph, self._graph_fp = g, fp
+                except Exception as e:   # a collective that cannot be captured here: nothing of the unit has run (the
+                    # library's host-side flags end a unit as they began it), so go on without graphs
+                    import sys
+                    print("[sharded] CUDA-graph capture of the step failed (%s): running without graphs" % e,
+                          file=sys.stderr, flush=True)
+                    self._graph, self._use_graph = None, False
+                    try:
+                        torch.cuda.synchronize()
+                    except Exception:
+                        pass
+            if self._graph is not None:
+                for _ in range(rest):
+                    self._graph.replay()
+            else:
+                for _ in range(rest):
+                    self._unit(main, True, torch)
         else:
             for _ in range(rest):
                 self._unit(main, True, torch)
