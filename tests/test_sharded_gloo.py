@@ -72,6 +72,7 @@ def _worker(rank, world, port, q, sensing):
         stepper.step(STEPS)
         st = _state(o)
         q.put((rank, {k: (v if isinstance(v, dict) else v.tolist()) for k, v in st.items()}))
+        dist.barrier()      # no rank tears the group down while the other is still inside a collective
     finally:
         dist.destroy_process_group()
 
