@@ -9,7 +9,13 @@ namespace {
 
 // ---- P3: one warp per cone; lanes take stencil cells; integer sums only (bit-exact) --------------------------
 // sense[c][s] = (n_s, Mx_s, My_s, Mz_s), M_s = sum over stencil offsets d of count_s(cell + d) * d   (reading A-12)
+#ifndef AXG_SENSE_STAGE
+#define AXG_SENSE_STAGE 0
+#endif
 __global__ void __launch_bounds__(256) k_sense(const AxgParams p) {
+#if AXG_SENSE_STAGE
+    __shared__ uint32_t s_stage[256][2];
+#endif
     const int lane = threadIdx.x & 31;
     const uint32_t warps_total = (gridDim.x * blockDim.x) >> 5;
     const uint32_t* __restrict__ cell_lo = p.cell_lo;
@@ -31,7 +37,18 @@ __global__ void __launch_bounds__(256) k_sense(const AxgParams p) {
             const int x = ci + dx, y = cj + dy, z = ck + dz;
             if (x < 0 || y < 0 || z < 0 || x >= (int)p.nx || y >= (int)p.ny || z >= (int)p.nz) continue;
             const uint32_t cell = axg_key_of_cell(p, (uint32_t)x, (uint32_t)y, (uint32_t)z);
+#if AXG_SENSE_STAGE
+            // north_star's form: the cell range staged in shared memory by cp.async (two 4-byte copies: the pair sits at an
+            // arbitrary 4-byte alignment), read back after the group has landed.  Measured against the direct loads below
+            // (profiles/r02_experiments.md §8): not faster -- the pair is used once, by the lane that asked for it.
+            const uint32_t sm = axg_smem_u32(&s_stage[threadIdx.x][0]);
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(sm), "l"(cell_lo + cell) : "memory");
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(sm + 4u), "l"(cell_lo + cell + 1) : "memory");
+            asm volatile("cp.async.wait_all;" ::: "memory");
+            const uint32_t a = s_stage[threadIdx.x][0], b = s_stage[threadIdx.x][1];
+#else
             const uint32_t a = __ldg(cell_lo + cell), b = __ldg(cell_lo + cell + 1);
+#endif
             if (p.single_species >= 0) {
                 const int cnt = (int)(b - a);
 #pragma unroll
